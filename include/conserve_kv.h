@@ -1,0 +1,296 @@
+/*
+ * conserve_kv.h — C ABI of libconserve_kv.so
+ *
+ * The data-parallel hot path under ConServe's conversation-level
+ * disaggregation (arxiv/paper_2606_01839): the memory-bound conversation tail
+ * that is pinned to one decoder, plus the one-shot KV handoff that brings a
+ * conversation's turn-1 prefill KV into that decoder's paged pool.
+ *
+ * Citations are "PAPER.md:N" = line N of the paper text, with the section.
+ * The paper describes no kernel and no layout (it names vLLM + LMCache,
+ * PAPER.md:213 §5.1); every layout below is this library's own and is
+ * restated, independently, by the CPU oracle under oracle/.
+ *
+ * Conventions
+ *  - Plain C ABI. Every call that can fail returns int: CSV_OK (0) or a
+ *    negative CSV_E_* code. A failed call changes nothing (no partial
+ *    allocation, no launch).
+ *  - The library NEVER allocates device memory. "d_" arguments are device
+ *    pointers owned by the caller (e.g. torch tensors' data_ptr()); "h_"
+ *    arguments are host pointers. `stream` is a cudaStream_t passed as void*.
+ *  - Kernel-launching calls enqueue on `stream` and return without
+ *    synchronising. Host-side calls (allocator, plan, place) are synchronous,
+ *    thread-compatible, not thread-safe.
+ *  - Supported shapes (anything else -> CSV_E_INVAL): bf16 (dtype 0),
+ *    block_size 16, head_dim in {64, 128}, num_kv_heads in {1, 2, 4, 8},
+ *    GQA group G = Hq / Hkv in {1, 2, 4, 8}.
+ *  - There is no CPU fallback: if no CUDA device / kernel image is usable the
+ *    launching calls return CSV_E_CUDA.
+ *
+ * Pool layout (one pool = one decoder's, or the prefiller's, KV memory)
+ *
+ *   A pool is an array of TILES.  tile(layer, block, kv, head) has index
+ *       ((layer * num_blocks + block) * 2 + kv) * Hkv + head        kv: 0 = K, 1 = V
+ *   and holds block_size * head_dim bf16 = the K (or V) rows of one KV head
+ *   for the 16 token slots of one block: 4 KiB at head_dim 128, 2 KiB at 64.
+ *   All tiles of one (layer, block) are contiguous (2 * Hkv tiles = 64 KiB at
+ *   the 8B / 70B shapes).
+ *
+ *   Inside a tile, element (slot, c), slot in [0,16), c in [0,head_dim):
+ *       half  = c / 64            (head_dim 64 has one half)
+ *       chunk = (c % 64) / 8      (a chunk = 8 bf16 = 16 bytes)
+ *       e     = c % 8
+ *       off   = half * (16 * 64) + slot * 64 + ((chunk ^ (slot & 7)) * 8) + e     [bf16 units]
+ *   i.e. each half is 16 rows of 128 bytes whose 16-byte chunks are XOR-ed
+ *   with the row index mod 8.  This is the image a TMA load with
+ *   SWIZZLE_128B would leave in shared memory; storing it in HBM means a
+ *   plain 1-D bulk copy (cp.async.bulk) of a tile lands ready for
+ *   bank-conflict-free ldmatrix / tensor-core use. The handoff writes it once
+ *   (§4 "transferred once"), every tail step reads it
+ *   (§2.1 "reading the full KV cache").
+ *
+ *   Token t of a conversation lives in block table[t / 16], slot t % 16; one
+ *   block table per conversation serves all layers.
+ *
+ * Staging message layout (the unit that crosses from prefiller to decoder)
+ *
+ *   For `tokens` tokens that will occupy conversation positions
+ *   [token_offset, token_offset + tokens): slot0 = token_offset % 16,
+ *   ntile_blocks = ceil((slot0 + tokens) / 16).  The message is the run of
+ *   tiles  [layer][tb][kv][head],  tb in [0, ntile_blocks), each in the pool's
+ *   intra-tile format; message token i sits in tb = (slot0 + i) / 16 at slot
+ *   (slot0 + i) % 16.  Slots of the message that carry no token are written
+ *   as zero by kv_pack and ignored by kv_unpack.
+ */
+#ifndef CONSERVE_KV_H_
+#define CONSERVE_KV_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CSV_OK        0
+#define CSV_E_INVAL  (-1)   /* bad argument, unsupported shape, misaligned pointer */
+#define CSV_E_NOMEM  (-2)   /* pool exhausted / workspace too small */
+#define CSV_E_CUDA   (-3)   /* a CUDA runtime call failed; see csv_last_cuda_error() */
+
+#define CSV_DTYPE_BF16 0
+#define CSV_BLOCK_SIZE 16
+
+typedef struct kv_pool  kv_pool_t;   /* host object; owns no device memory */
+typedef struct csv_plan csv_plan_t;  /* host object + pointers into caller workspace */
+
+/* Shape of a pool / of a conversation's KV. */
+typedef struct {
+    int32_t num_layers;    /* NL */
+    int32_t num_blocks;    /* blocks in the pool (ignored by kv_pack / kv_staging_bytes) */
+    int32_t block_size;    /* must be 16 */
+    int32_t num_kv_heads;  /* Hkv */
+    int32_t head_dim;      /* d: 64 or 128 */
+    int32_t dtype;         /* CSV_DTYPE_BF16 */
+} kv_pool_desc;
+
+/* Shape of an attention call. */
+typedef struct {
+    int32_t num_q_heads;   /* Hq, a multiple of Hkv */
+    int32_t num_kv_heads;  /* Hkv */
+    int32_t head_dim;      /* d */
+    int32_t block_size;    /* 16 */
+} csv_attn_shape;
+
+/* cudaError_t of the last failing CUDA call made by this library (0 if none). */
+int csv_last_cuda_error(void);
+/* Library version string, static storage. */
+const char* csv_version(void);
+
+/* ------------------------------------------------------------------------
+ * a1. Block-table allocator (host only).  PAPER.md:11 §1 "a KV cache that only
+ * grows"; §4.2: per-decoder *active* KV occupancy, decremented on
+ * conversation termination; §5.1: a decoder holds ~300k tokens.
+ * ---------------------------------------------------------------------- */
+
+/* Bytes a pool of this shape occupies: NL * num_blocks * 2 * Hkv * 16 * d * 2. */
+size_t kv_pool_bytes(const kv_pool_desc* desc);
+
+/* Wrap caller memory as a pool.  d_base: device pointer, 128-byte aligned,
+ * `bytes` >= kv_pool_bytes(desc).  The free list starts as 0,1,...,num_blocks-1.
+ * The pool contents are not touched.  *out receives the handle. */
+int kv_pool_create(const kv_pool_desc* desc, void* d_base, size_t bytes, kv_pool_t** out);
+/* Frees the host object only. */
+int kv_pool_destroy(kv_pool_t* pool);
+/* Install a caller-chosen order of the currently free blocks: `order` must be
+ * a permutation of exactly the free ids (n = number free).  Blocks are then
+ * handed out order[0], order[1], ...  (how the harness gets "a shuffled
+ * free-block list"). */
+int kv_pool_set_free_order(kv_pool_t* pool, const int32_t* h_order, int32_t n);
+/* Pop n ids in free-list order into h_out_ids.  All-or-nothing: CSV_E_NOMEM
+ * and no change if fewer than n are free.  n = 0 is OK.  Growing a
+ * conversation = another call, appended to the caller's table. */
+int kv_alloc_blocks(kv_pool_t* pool, int32_t n, int32_t* h_out_ids);
+/* Conversation termination.  Ids are pushed back at the tail of
+ * the free list in the order given.  Out-of-range id, double free, or a
+ * duplicate inside `h_ids` -> CSV_E_INVAL and no change. */
+int kv_free_blocks(kv_pool_t* pool, const int32_t* h_ids, int32_t n);
+/* Active occupancy in blocks / pool size / free count (negative on NULL). */
+int32_t kv_pool_used_blocks(const kv_pool_t* pool);
+int32_t kv_pool_num_blocks(const kv_pool_t* pool);
+int32_t kv_pool_free_blocks(const kv_pool_t* pool);
+/* Copy the pool's shape into *out. */
+int kv_pool_get_desc(const kv_pool_t* pool, kv_pool_desc* out);
+
+/* ------------------------------------------------------------------------
+ * a6. Placement (host only).  PAPER.md:178 §4.2: "binds the conversation to
+ * the decoder replica with the lowest current KV cache occupancy. The binding
+ * is persistent"; §1: a saturated decoder is skipped ("routes the
+ * next conversation elsewhere rather than migrating one already placed").
+ * Occupancy = used / total blocks (compared exactly, as cross-multiplied
+ * integers); ties -> lowest index; pools with fewer than need_blocks free are
+ * skipped; none fits -> CSV_E_NOMEM.  Never moves anything.
+ * ---------------------------------------------------------------------- */
+int csv_place(const kv_pool_t* const* pools, int32_t n_pools, int32_t need_blocks, int32_t* out_idx);
+
+/* Provisioning, §4.1: R* = T_p / L_in; Eq. 1  N*T_d >= R*L_d;
+ * Eq. 2  N*B >= R*W.  Writes R*, the two real-valued lower bounds on N at
+ * R = R*, and the smallest integer N satisfying both.  Any non-positive
+ * input -> CSV_E_INVAL.  Worked example PAPER.md:209: 25k, 15k, 1k, 1k -> 1.67. */
+int csv_provision(double T_p, double L_in, double T_d, double L_d, double B, double W,
+                  double* out_rate, double* out_n_throughput, double* out_n_memory, int32_t* out_n);
+
+/* ------------------------------------------------------------------------
+ * a2 / a3. One-shot KV handoff.  PAPER.md:150 §4: "the resulting KV cache is
+ * transferred once to the bound decoder"; §3.1 / Fig. 3: cost
+ * linear in tokens.  Pure 16-byte moves: bit-exact for any bit pattern.
+ * ---------------------------------------------------------------------- */
+
+/* Bytes of the staging message for `tokens` tokens landing at token_offset
+ * (see layout above).  0 if tokens <= 0 or the shape is unsupported. */
+size_t kv_staging_bytes(const kv_pool_desc* shape, int32_t tokens, int32_t token_offset);
+
+/* One conversation's handoff.  Source is contiguous and token-major, as a
+ * prefiller holds it: d_k, d_v each [NL][tokens][Hkv][d] bf16, 16-byte
+ * aligned.  d_staging: >= kv_staging_bytes(...), 128-byte aligned; every byte
+ * of the message is written (unused slots as zero). */
+int kv_pack(const kv_pool_desc* shape, const void* d_k, const void* d_v, int32_t tokens,
+            int32_t token_offset, void* d_staging, void* stream);
+
+/* Scatter a message into `dst` through the conversation's block table.
+ * Writes conversation positions [token_offset, token_offset + tokens);
+ * token_offset = 0 for the handoff, = P for a tail append.  d_block_ids: the
+ * conversation's whole table on the device (n_ids entries, n_ids >=
+ * ceil((token_offset + tokens) / 16), else CSV_E_INVAL before any launch).
+ * Slots not addressed are NOT written.  Destination blocks must be exclusive
+ * to this conversation.  The pool's shape must equal the message's. */
+int kv_unpack(kv_pool_t* dst, const void* d_staging, int32_t tokens, int32_t token_offset,
+              const int32_t* d_block_ids, int32_t n_ids, void* stream);
+
+/* Batched forms: n conversations in as few launches as possible (arrays are
+ * host arrays of length n; device pointers inside).  Entries with tokens = 0
+ * are skipped.  Semantics per entry identical to the single calls. */
+int kv_pack_batch(const kv_pool_desc* shape, int32_t n, const void* const* h_d_k,
+                  const void* const* h_d_v, const int32_t* h_tokens, const int32_t* h_token_offsets,
+                  void* const* h_d_staging, void* stream);
+int kv_unpack_batch(kv_pool_t* dst, int32_t n, const void* const* h_d_staging,
+                    const int32_t* h_tokens, const int32_t* h_token_offsets,
+                    const int32_t* const* h_d_block_ids, const int32_t* h_n_ids, void* stream);
+
+/* Tail-step KV append ("appending one new entry"; PAPER.md:94
+ * "only calculating new KV cache entries for the appended tokens"): writes the
+ * new tokens' K/V of a whole batch straight from token-major projections into
+ * the pool — the composition kv_unpack(kv_pack(.)) without the staging round
+ * trip.  d_k_new, d_v_new: [NL][total_q][Hkv][d] bf16 where total_q = sum of
+ * the plan's q_lens; conversation b's rows start at sum_{b'<b} q_len[b'] and go
+ * to positions [kv_len[b] - q_len[b], kv_len[b]).  d_block_tables:
+ * [batch][max_blocks] int32. */
+int kv_append_tokens(kv_pool_t* dst, const csv_plan_t* plan, const void* d_k_new, const void* d_v_new,
+                     const int32_t* d_block_tables, int32_t max_blocks, void* stream);
+
+/* ------------------------------------------------------------------------
+ * Step plan (host).  Lengths are per step, not per layer: one plan serves all
+ * layers of a step and both attention calls.  Conversation b has q_len[b] new
+ * query rows and kv_len[b] tokens in the cache INCLUDING those rows' own K/V
+ * (the caller writes them first; a token attends to itself).  q_len 1 =
+ * decode row, q_len m > 1 = appended chunk with prefix P = kv_len - m.
+ *
+ * Split-K: the flattened (conversation, block) stream of the q_len = 1 rows is
+ * cut into one contiguous share per CTA, and each share into partitions of at
+ * most max_partition_tokens tokens (a multiple of 16; 0 = default 2048) that
+ * never cross a conversation.  The schedule depends only on the lengths, so
+ * results are bit-identical under any block permutation and from run to run.
+ * ---------------------------------------------------------------------- */
+
+/* Device workspace the plan needs (partials, work lists), for these lengths. */
+size_t csv_plan_workspace_bytes(const csv_attn_shape* shape, const int32_t* h_q_lens,
+                                const int32_t* h_kv_lens, int32_t batch, int32_t max_partition_tokens);
+/* Builds the plan and enqueues the copy of its work lists into d_workspace
+ * (128-byte aligned) on `stream`.  q_len[b] must be in [0, kv_len[b]];
+ * q_len = 0 rows are inert.  The plan may be used on that stream (or after
+ * synchronising with it) until destroyed; the workspace must outlive it. */
+int csv_plan_create(const csv_attn_shape* shape, const int32_t* h_q_lens, const int32_t* h_kv_lens,
+                    int32_t batch, int32_t max_partition_tokens, void* d_workspace, size_t ws_bytes,
+                    void* stream, csv_plan_t** out);
+int csv_plan_destroy(csv_plan_t* plan);
+/* Introspection for tests / bench: number of decode work items (partitions),
+ * number of decode rows, of append chunks, sum of append q rows, CTAs used. */
+int csv_plan_info(const csv_plan_t* plan, int32_t* n_decode_items, int32_t* n_decode_rows,
+                  int32_t* n_append_chunks, int32_t* n_append_rows, int32_t* decode_grid);
+
+/* ------------------------------------------------------------------------
+ * a4. paged_decode_attn.  PAPER.md:50 §2.1: decode "generates each subsequent
+ * token by reading the full KV cache"; §3.2 / Fig. 4: the
+ * tail is bandwidth-bound.  For every conversation b of the plan with
+ * q_len[b] = 1 and every query head h (KV head h / G):
+ *     s_j = q . K_j / sqrt(d),  j in [0, kv_len[b])
+ *     O   = sum_j softmax(s)_j V_j          (bf16, round-to-nearest-even)
+ *     LSE = ln sum_j exp(s_j)               (fp32, natural log)
+ * kv_len = 0 -> O = 0, LSE = -inf.  bf16 inputs, fp32 scores / softmax /
+ * accumulation; softmax weights are rounded to bf16 for the PV product.
+ *
+ * d_q:   [batch][Hq][d] bf16 (row b is read only if q_len[b] = 1), 16-byte aligned.
+ * d_block_tables: [batch][max_blocks] int32; entries past ceil(kv_len/16) are never read.
+ * d_out: [batch][Hq][d] bf16;  d_lse: [batch][Hq] fp32.  Rows with q_len != 1 are untouched.
+ * Pool slots past kv_len in the last block may hold anything (NaN patterns included).
+ * ---------------------------------------------------------------------- */
+int paged_decode_attn(const csv_plan_t* plan, const kv_pool_t* pool, int32_t layer, const void* d_q,
+                      const int32_t* d_block_tables, int32_t max_blocks, void* d_out, float* d_lse,
+                      void* stream);
+
+/* ------------------------------------------------------------------------
+ * a5. append_prefill_attn.  PAPER.md:94 §3.1: "relatively small prompts are
+ * appended to the whole history context ... only calculating new KV cache
+ * entries for the appended tokens"; §2.2: appends run on the
+ * decoder holding the cached prefix.  For every conversation b with
+ * q_len[b] = m > 1: query row i (position P + i, P = kv_len - m) attends to
+ * keys 0 .. P + i (prefix fully visible, causal inside the chunk, diagonal
+ * included).  Same softmax, outputs and precision as paged_decode_attn.
+ *
+ * d_q / d_out: [total_q][Hq][d] bf16 with total_q = sum of ALL q_lens of the
+ * plan (decode rows included, in batch order; decode rows are skipped here).
+ * d_lse: [total_q][Hq] fp32.
+ * ---------------------------------------------------------------------- */
+int append_prefill_attn(const csv_plan_t* plan, const kv_pool_t* pool, int32_t layer, const void* d_q,
+                        const int32_t* d_block_tables, int32_t max_blocks, void* d_out, float* d_lse,
+                        void* stream);
+
+/* ------------------------------------------------------------------------
+ * End-to-end convenience with HOST buffers (what bench.py's "e2e" times): one
+ * decode tail step of one layer.  Plans from the host lengths, copies
+ * h_q, h_k_new, h_v_new ([batch][Hq|Hkv][d] bf16, one new token per
+ * conversation, already counted in h_kv_lens) and h_block_tables to the
+ * device workspace, runs kv_append_tokens + paged_decode_attn, copies O and
+ * LSE back to h_out / h_lse and synchronises `stream`.
+ * d_workspace: >= csv_tail_step_host_workspace_bytes(...), 128-byte aligned.
+ * ---------------------------------------------------------------------- */
+size_t csv_tail_step_host_workspace_bytes(const csv_attn_shape* shape, const int32_t* h_kv_lens,
+                                          int32_t batch, int32_t max_blocks, int32_t max_partition_tokens);
+int csv_tail_step_host(kv_pool_t* pool, int32_t layer, const csv_attn_shape* shape, int32_t batch,
+                       const int32_t* h_kv_lens, const void* h_q, const void* h_k_new, const void* h_v_new,
+                       const int32_t* h_block_tables, int32_t max_blocks, int32_t max_partition_tokens,
+                       void* d_workspace, size_t ws_bytes, void* h_out, float* h_lse, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CONSERVE_KV_H_ */
