@@ -227,7 +227,10 @@ size_t csv_plan_workspace_bytes(const csv_attn_shape* shape, const int32_t* h_q_
 /* Builds the plan and enqueues the copy of its work lists into d_workspace
  * (128-byte aligned) on `stream`.  q_len[b] must be in [0, kv_len[b]];
  * q_len = 0 rows are inert.  The plan may be used on that stream (or after
- * synchronising with it) until destroyed; the workspace must outlive it. */
+ * synchronising with it) until destroyed; the workspace must outlive it.
+ * d_workspace = NULL builds a host-only plan (no CUDA call): good for
+ * csv_plan_info / csv_plan_*_items, refused (CSV_E_INVAL) by the attention calls.
+ * ws_bytes too small -> CSV_E_NOMEM. */
 int csv_plan_create(const csv_attn_shape* shape, const int32_t* h_q_lens, const int32_t* h_kv_lens,
                     int32_t batch, int32_t max_partition_tokens, void* d_workspace, size_t ws_bytes,
                     void* stream, csv_plan_t** out);
@@ -236,6 +239,19 @@ int csv_plan_destroy(csv_plan_t* plan);
  * number of decode rows, of append chunks, sum of append q rows, CTAs used. */
 int csv_plan_info(const csv_plan_t* plan, int32_t* n_decode_items, int32_t* n_decode_rows,
                   int32_t* n_append_chunks, int32_t* n_append_rows, int32_t* decode_grid);
+/* Sum of the plan's q_lens (rows of d_q / d_out for append_prefill_attn); -1 on NULL. */
+int32_t csv_plan_total_q(const csv_plan_t* plan);
+/* Copies the decode work list for inspection (host tests): item i is 8 int32
+ * {conv, kv_head, blk_begin, blk_end, kv_len, partial, direct, 0} at h_out[8*i];
+ * h_worker_begin[w] .. h_worker_begin[w+1] are the items of warp-worker w
+ * (decode_grid * 8 workers).  Either output may be NULL.  Returns the item count. */
+int32_t csv_plan_decode_items(const csv_plan_t* plan, int32_t* h_out, int32_t max_items,
+                              int32_t* h_worker_begin, int32_t max_workers_plus_1);
+/* Same for the append work list: item i is 12 int32 {conv, kv_head, row_begin,
+ * q_start, m, kv_len, blk_begin, blk_end, partial, direct, 0, 0}; rows are the
+ * m * G query rows of a chunk stacked token-major (row = token * G + head_in_group),
+ * in tiles of 64.  Returns the item count. */
+int32_t csv_plan_append_items(const csv_plan_t* plan, int32_t* h_out, int32_t max_items);
 
 /* ------------------------------------------------------------------------
  * a4. paged_decode_attn.  PAPER.md:50 §2.1: decode "generates each subsequent

@@ -1,0 +1,237 @@
+// api.cu — the extern "C" entry points of include/conserve_kv.h that touch CUDA: argument
+// validation, plan upload, launches, and the host-buffer tail step.  No kernels here.
+#include <new>
+
+#include "common.cuh"
+#include "internal.h"
+
+static thread_local int g_last_cuda_error = 0;
+int csv_set_cuda_error(int err) {
+    g_last_cuda_error = err;
+    return CSV_E_CUDA;
+}
+
+int csv_query_num_sms() {
+    static int cached = -1;
+    if (cached > 0) return cached;
+    int dev = 0, n = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess &&
+        cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0) {
+        cached = n;
+        return n;
+    }
+    (void)cudaGetLastError();
+    return 148;   // B200; lets the planner run on a box without a GPU (host tests)
+}
+
+static bool aligned(const void* p, size_t a) { return ((uintptr_t)p & (a - 1)) == 0; }
+
+static bool same_shape(const kv_pool_desc& a, const csv_attn_shape& s) {
+    return a.num_kv_heads == s.num_kv_heads && a.head_dim == s.head_dim && a.block_size == s.block_size;
+}
+
+extern "C" {
+
+int csv_last_cuda_error(void) { return g_last_cuda_error; }
+
+size_t kv_staging_bytes(const kv_pool_desc* shape, int32_t tokens, int32_t token_offset) {
+    if (!csv_shape_ok(shape, false) || tokens <= 0 || token_offset < 0) return 0;
+    const int slot0 = token_offset & 15;
+    const size_t ntb = (size_t)(slot0 + tokens + 15) / 16;
+    return (size_t)shape->num_layers * ntb * 2u * shape->num_kv_heads * csv_tile_bytes(shape->head_dim);
+}
+
+int kv_pack_batch(const kv_pool_desc* shape, int32_t n, const void* const* h_d_k, const void* const* h_d_v,
+                  const int32_t* h_tokens, const int32_t* h_token_offsets, void* const* h_d_staging, void* stream) {
+    if (!csv_shape_ok(shape, false) || n < 0) return CSV_E_INVAL;
+    if (n > 0 && (!h_d_k || !h_d_v || !h_tokens || !h_token_offsets || !h_d_staging)) return CSV_E_INVAL;
+    for (int i = 0; i < n; ++i) {
+        if (h_tokens[i] < 0 || h_token_offsets[i] < 0) return CSV_E_INVAL;
+        if (h_tokens[i] == 0) continue;
+        if (!h_d_k[i] || !h_d_v[i] || !h_d_staging[i]) return CSV_E_INVAL;
+        if (!aligned(h_d_k[i], 16) || !aligned(h_d_v[i], 16) || !aligned(h_d_staging[i], 128)) return CSV_E_INVAL;
+    }
+    return launch_pack(*shape, n, h_d_k, h_d_v, h_tokens, h_token_offsets, h_d_staging, stream);
+}
+
+int kv_pack(const kv_pool_desc* shape, const void* d_k, const void* d_v, int32_t tokens, int32_t token_offset,
+            void* d_staging, void* stream) {
+    if (tokens <= 0) return CSV_E_INVAL;
+    return kv_pack_batch(shape, 1, &d_k, &d_v, &tokens, &token_offset, &d_staging, stream);
+}
+
+int kv_unpack_batch(kv_pool_t* dst, int32_t n, const void* const* h_d_staging, const int32_t* h_tokens,
+                    const int32_t* h_token_offsets, const int32_t* const* h_d_block_ids, const int32_t* h_n_ids,
+                    void* stream) {
+    if (!dst || n < 0) return CSV_E_INVAL;
+    if (n > 0 && (!h_d_staging || !h_tokens || !h_token_offsets || !h_d_block_ids || !h_n_ids)) return CSV_E_INVAL;
+    for (int i = 0; i < n; ++i) {
+        if (h_tokens[i] < 0 || h_token_offsets[i] < 0) return CSV_E_INVAL;
+        if (h_tokens[i] == 0) continue;
+        if (!h_d_staging[i] || !h_d_block_ids[i] || !aligned(h_d_staging[i], 128) || !aligned(h_d_block_ids[i], 4))
+            return CSV_E_INVAL;
+        const int64_t need = ((int64_t)h_token_offsets[i] + h_tokens[i] + 15) / 16;
+        if ((int64_t)h_n_ids[i] < need) return CSV_E_INVAL;
+    }
+    return launch_unpack(dst, n, h_d_staging, h_tokens, h_token_offsets, h_d_block_ids, stream);
+}
+
+int kv_unpack(kv_pool_t* dst, const void* d_staging, int32_t tokens, int32_t token_offset, const int32_t* d_block_ids,
+              int32_t n_ids, void* stream) {
+    if (tokens <= 0) return CSV_E_INVAL;
+    return kv_unpack_batch(dst, 1, &d_staging, &tokens, &token_offset, &d_block_ids, &n_ids, stream);
+}
+
+int csv_plan_create(const csv_attn_shape* shape, const int32_t* h_q_lens, const int32_t* h_kv_lens, int32_t batch,
+                    int32_t max_partition_tokens, void* d_workspace, size_t ws_bytes, void* stream, csv_plan_t** out) {
+    if (!out) return CSV_E_INVAL;
+    int err;
+    csv_plan* p = csv_plan_build_host(shape, h_q_lens, h_kv_lens, batch, max_partition_tokens, &err);
+    if (!p) return err;
+    if (d_workspace) {
+        if (!aligned(d_workspace, 128)) {
+            delete p;
+            return CSV_E_INVAL;
+        }
+        if (ws_bytes < p->lay.total) {
+            delete p;
+            return CSV_E_NOMEM;
+        }
+        p->d_ws = (uint8_t*)d_workspace;
+        if (!p->h_image.empty()) {
+            // pageable source: the runtime stages it before returning, so h_image may be reused freely
+            cudaError_t e = cudaMemcpyAsync(d_workspace, p->h_image.data(), p->h_image.size(), cudaMemcpyHostToDevice,
+                                            (cudaStream_t)stream);
+            if (e != cudaSuccess) {
+                delete p;
+                return csv_set_cuda_error((int)e);
+            }
+        }
+    }
+    *out = p;
+    return CSV_OK;
+}
+
+static int check_attn_args(const csv_plan_t* plan, const kv_pool_t* pool, int32_t layer, const void* d_q,
+                           const int32_t* d_block_tables, int32_t max_blocks, void* d_out, float* d_lse) {
+    if (!plan || !pool || !plan->d_ws) return CSV_E_INVAL;
+    if (!same_shape(pool->desc, plan->shape)) return CSV_E_INVAL;
+    if (layer < 0 || layer >= pool->desc.num_layers) return CSV_E_INVAL;
+    if (!d_q || !d_block_tables || !d_out || !d_lse || !aligned(d_q, 16) || !aligned(d_out, 16) || !aligned(d_lse, 4))
+        return CSV_E_INVAL;
+    int64_t need = 0;
+    for (int b = 0; b < plan->batch; ++b)
+        if (plan->q_lens[(size_t)b] > 0) need = std::max<int64_t>(need, ((int64_t)plan->kv_lens[(size_t)b] + 15) / 16);
+    if ((int64_t)max_blocks < need) return CSV_E_INVAL;
+    return CSV_OK;
+}
+
+int paged_decode_attn(const csv_plan_t* plan, const kv_pool_t* pool, int32_t layer, const void* d_q,
+                      const int32_t* d_block_tables, int32_t max_blocks, void* d_out, float* d_lse, void* stream) {
+    const int rc = check_attn_args(plan, pool, layer, d_q, d_block_tables, max_blocks, d_out, d_lse);
+    if (rc != CSV_OK) return rc;
+    return launch_decode(plan, pool, layer, d_q, d_block_tables, max_blocks, d_out, d_lse, stream);
+}
+
+int append_prefill_attn(const csv_plan_t* plan, const kv_pool_t* pool, int32_t layer, const void* d_q,
+                        const int32_t* d_block_tables, int32_t max_blocks, void* d_out, float* d_lse, void* stream) {
+    const int rc = check_attn_args(plan, pool, layer, d_q, d_block_tables, max_blocks, d_out, d_lse);
+    if (rc != CSV_OK) return rc;
+    return launch_append_attn(plan, pool, layer, d_q, d_block_tables, max_blocks, d_out, d_lse, stream);
+}
+
+int kv_append_tokens(kv_pool_t* dst, const csv_plan_t* plan, const void* d_k_new, const void* d_v_new,
+                     const int32_t* d_block_tables, int32_t max_blocks, void* stream) {
+    if (!dst || !plan || !plan->d_ws || !same_shape(dst->desc, plan->shape)) return CSV_E_INVAL;
+    if (plan->total_q == 0) return CSV_OK;
+    if (!d_k_new || !d_v_new || !d_block_tables || !aligned(d_k_new, 16) || !aligned(d_v_new, 16)) return CSV_E_INVAL;
+    int64_t need = 0;
+    for (int b = 0; b < plan->batch; ++b)
+        if (plan->q_lens[(size_t)b] > 0) need = std::max<int64_t>(need, ((int64_t)plan->kv_lens[(size_t)b] + 15) / 16);
+    if ((int64_t)max_blocks < need) return CSV_E_INVAL;
+    return launch_append_tokens(dst, plan, d_k_new, d_v_new, d_block_tables, max_blocks, stream);
+}
+
+// ---- host-buffer tail step (bench.py "e2e") ---------------------------------------------------
+struct TailLayout {
+    size_t plan, q, k, v, tables, out, lse, total;
+};
+static TailLayout tail_layout(const csv_attn_shape* s, int batch, int max_blocks, size_t plan_bytes) {
+    TailLayout L;
+    size_t off = 0;
+    auto take = [&](size_t b) {
+        const size_t at = off;
+        off = (off + b + 127) / 128 * 128;
+        return at;
+    };
+    L.plan = take(plan_bytes);
+    L.q = take((size_t)batch * s->num_q_heads * s->head_dim * 2);
+    L.k = take((size_t)batch * s->num_kv_heads * s->head_dim * 2);
+    L.v = take((size_t)batch * s->num_kv_heads * s->head_dim * 2);
+    L.tables = take((size_t)batch * max_blocks * 4);
+    L.out = take((size_t)batch * s->num_q_heads * s->head_dim * 2);
+    L.lse = take((size_t)batch * s->num_q_heads * 4);
+    L.total = off;
+    return L;
+}
+
+size_t csv_tail_step_host_workspace_bytes(const csv_attn_shape* shape, const int32_t* h_kv_lens, int32_t batch,
+                                          int32_t max_blocks, int32_t max_partition_tokens) {
+    if (!shape || batch <= 0 || max_blocks <= 0 || !h_kv_lens) return 0;
+    std::vector<int32_t> ones((size_t)batch, 1);
+    const size_t pb = csv_plan_workspace_bytes(shape, ones.data(), h_kv_lens, batch, max_partition_tokens);
+    if (pb == 0) return 0;
+    return tail_layout(shape, batch, max_blocks, pb).total;
+}
+
+int csv_tail_step_host(kv_pool_t* pool, int32_t layer, const csv_attn_shape* shape, int32_t batch,
+                       const int32_t* h_kv_lens, const void* h_q, const void* h_k_new, const void* h_v_new,
+                       const int32_t* h_block_tables, int32_t max_blocks, int32_t max_partition_tokens, void* d_workspace,
+                       size_t ws_bytes, void* h_out, float* h_lse, void* stream) {
+    if (!pool || !shape || batch <= 0 || !h_kv_lens || !h_q || !h_k_new || !h_v_new || !h_block_tables || !h_out ||
+        !h_lse || !d_workspace || !aligned(d_workspace, 128) || max_blocks <= 0)
+        return CSV_E_INVAL;
+    std::vector<int32_t> ones((size_t)batch, 1);
+    const size_t pb = csv_plan_workspace_bytes(shape, ones.data(), h_kv_lens, batch, max_partition_tokens);
+    if (pb == 0) return CSV_E_INVAL;
+    const TailLayout L = tail_layout(shape, batch, max_blocks, pb);
+    if (ws_bytes < L.total) return CSV_E_NOMEM;
+    uint8_t* ws = (uint8_t*)d_workspace;
+    cudaStream_t st = (cudaStream_t)stream;
+    csv_plan_t* plan = nullptr;
+    int rc = csv_plan_create(shape, ones.data(), h_kv_lens, batch, max_partition_tokens, ws + L.plan, pb, stream, &plan);
+    if (rc != CSV_OK) return rc;
+    const size_t qb = (size_t)batch * shape->num_q_heads * shape->head_dim * 2;
+    const size_t kb = (size_t)batch * shape->num_kv_heads * shape->head_dim * 2;
+    cudaError_t e;
+    if ((e = cudaMemcpyAsync(ws + L.q, h_q, qb, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(ws + L.k, h_k_new, kb, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(ws + L.v, h_v_new, kb, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(ws + L.tables, h_block_tables, (size_t)batch * max_blocks * 4, cudaMemcpyHostToDevice, st)) !=
+            cudaSuccess) {
+        csv_plan_destroy(plan);
+        return csv_set_cuda_error((int)e);
+    }
+    // the new token's K/V go to `layer` of the pool: view that layer as a 1-layer pool
+    kv_pool layer_view = *pool;
+    layer_view.desc.num_layers = 1;
+    layer_view.d_base = pool->d_base + (size_t)layer * pool->desc.num_blocks * 2 * pool->desc.num_kv_heads *
+                                           csv_tile_bytes(pool->desc.head_dim);
+    if (layer < 0 || layer >= pool->desc.num_layers) rc = CSV_E_INVAL;
+    if (rc == CSV_OK)
+        rc = kv_append_tokens(&layer_view, plan, ws + L.k, ws + L.v, (const int32_t*)(ws + L.tables), max_blocks, stream);
+    if (rc == CSV_OK)
+        rc = paged_decode_attn(plan, &layer_view, 0, ws + L.q, (const int32_t*)(ws + L.tables), max_blocks, ws + L.out,
+                               (float*)(ws + L.lse), stream);
+    if (rc == CSV_OK) {
+        if ((e = cudaMemcpyAsync(h_out, ws + L.out, qb, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
+            (e = cudaMemcpyAsync(h_lse, ws + L.lse, (size_t)batch * shape->num_q_heads * 4, cudaMemcpyDeviceToHost, st)) !=
+                cudaSuccess ||
+            (e = cudaStreamSynchronize(st)) != cudaSuccess)
+            rc = csv_set_cuda_error((int)e);
+    }
+    csv_plan_destroy(plan);
+    return rc;
+}
+
+}   // extern "C"

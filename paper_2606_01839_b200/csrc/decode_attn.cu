@@ -1,0 +1,291 @@
+// decode_attn.cu — paged_decode_attn (a4): split-K flash-decoding over block tables with GQA
+// head grouping and a log-sum-exp merge.  PAPER.md:50 §2.1: decode "generates each subsequent
+// token by reading the full KV cache"; §3.2: the tail is bandwidth-bound.
+//
+// Roofline: HBM.  Algorithmic bytes = sum_b kv_len_b * Hkv * d * 2 * 2 per layer.
+//
+// Design (sm_100a):
+//  * The unit of execution is a WARP, not a CTA.  Every warp of the grid is an independent
+//    worker with a private ring of STAGES x (K tile + V tile) in shared memory, private
+//    mbarriers and its own contiguous share of the flattened (conversation, KV head, block)
+//    stream (plan.cpp).  No __syncthreads anywhere; a long conversation never holds a CTA.
+//  * Lane 0 feeds the ring with 1-D bulk copies (cp.async.bulk, SASS UBLKCP): one 4 KiB K
+//    tile and one 4 KiB V tile per block, each contiguous in HBM and already in the 128-byte
+//    XOR-swizzled image ldmatrix wants (pool layout, conserve_kv.h).  8 warps x 3 stages x
+//    8 KiB = 192 KiB in flight per SM, well past the ~45 KiB/SM Little's law asks for.
+//  * The G query heads of the group are the (zero-padded) M rows of mma.sync.m16n8k16: one
+//    K/V tile read serves all G heads.  CUDA-core FMAs would need 2*d*(G+1) lane-ops per
+//    512 B of KV, 68-99 % of the FP32 issue rate at G = 8; HMMA makes
+//    the arithmetic ~8 % of issue slots so the kernel stays on the HBM roofline.
+//  * Online softmax in fp32 in the log2 domain; P rounded to bf16 for the PV product; each
+//    partition leaves (o, m, l) fp32 partials, merged in a fixed order by merge_kernel
+//    (deterministic, no float atomics).  Single-partition (conversation, head) pairs write
+//    O / LSE directly.
+#include <math.h>
+
+#include "common.cuh"
+#include "internal.h"
+
+namespace {
+
+struct DecodeParams {
+    const DecodeItem* items;
+    const int32_t* worker_begin;
+    const uint8_t* pool_layer;   // first tile of this layer
+    const uint16_t* q;
+    const int32_t* tables;
+    uint16_t* out;
+    float* lse;
+    float* po;
+    float* pml;
+    int32_t max_blocks, Hq, Hkv, G;
+    float scale_log2;
+};
+
+template <int D, int STAGES>
+__global__ void __launch_bounds__(kDecodeWarps * 32, 1) decode_kernel(const __grid_constant__ DecodeParams p) {
+    constexpr int TB = 16 * D * 2;   // tile bytes
+    constexpr int KS = D / 16;       // k-steps of Q K^T
+    constexpr int NT = D / 8;        // n-tiles of P V
+    extern __shared__ __align__(1024) uint8_t smem[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int worker = blockIdx.x * kDecodeWarps + warp;
+    uint8_t* ring = smem + (size_t)warp * STAGES * 2 * TB;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)kDecodeWarps * STAGES * 2 * TB) + warp * STAGES;
+    if (lane == 0) {
+        for (int s = 0; s < STAGES; ++s) mbar_init(&bars[s], 1);
+        fence_mbar_init();
+    }
+    __syncwarp();
+
+    const int G = p.G;
+    const int row = lane >> 2, t4 = lane & 3;
+    const size_t kv_stride = (size_t)p.Hkv * TB;   // K tile -> V tile of the same head
+    const size_t blk_stride = 2 * kv_stride;
+
+    // per-lane ldmatrix offsets inside a tile (see conserve_kv.h "Inside a tile")
+    const int mi = lane >> 3, r8 = lane & 7;
+    const uint32_t k_lane_off = (uint32_t)((r8 + 8 * (mi >> 1)) * 128 + (((mi & 1) ^ r8) << 4));
+    const uint32_t v_lane_off = (uint32_t)((r8 + 8 * (mi & 1)) * 128 + (((mi >> 1) ^ r8) << 4));
+    const uint32_t ring_u32 = smem_u32(ring);
+
+    uint32_t cnt = 0;   // blocks consumed so far by this warp (ring position)
+    const int item_begin = __ldg(p.worker_begin + worker), item_end = __ldg(p.worker_begin + worker + 1);
+    for (int ii = item_begin; ii < item_end; ++ii) {
+        const int4 i0 = __ldg(reinterpret_cast<const int4*>(p.items + ii));
+        const int4 i1 = __ldg(reinterpret_cast<const int4*>(p.items + ii) + 1);
+        const int conv = i0.x, head = i0.y, blk_begin = i0.z, blk_end = i0.w;
+        const int kv_len = i1.x, partial = i1.y, direct = i1.z;
+        const int nblk = blk_end - blk_begin;
+        const int32_t* tab = p.tables + (size_t)conv * p.max_blocks + blk_begin;
+        int ids_cur = lane < nblk ? __ldg(tab + lane) : 0;
+        int ids_nxt = 32 + lane < nblk ? __ldg(tab + 32 + lane) : 0;
+        int grp_cur = 0;
+
+        // Q fragments: row `row` of the group (zero beyond G); rows 8..15 of the MMA are zero
+        uint32_t qa[KS][2];
+        {
+            const uint16_t* qrow = p.q + ((size_t)conv * p.Hq + (size_t)head * G + row) * D;
+#pragma unroll
+            for (int ks = 0; ks < KS; ++ks) {
+                qa[ks][0] = row < G ? *reinterpret_cast<const uint32_t*>(qrow + ks * 16 + 2 * t4) : 0u;
+                qa[ks][1] = row < G ? *reinterpret_cast<const uint32_t*>(qrow + ks * 16 + 8 + 2 * t4) : 0u;
+            }
+        }
+        float o[NT][2];
+#pragma unroll
+        for (int n = 0; n < NT; ++n) o[n][0] = o[n][1] = 0.f;
+        float m_run = -INFINITY, l_run = 0.f;
+
+        const uint8_t* head_base = p.pool_layer + (size_t)head * TB;
+        const uint32_t cnt0 = cnt;
+        // prologue: fill the ring
+        const int npro = nblk < STAGES ? nblk : STAGES;
+        for (int j = 0; j < npro; ++j) {
+            const int id = __shfl_sync(0xffffffffu, ids_cur, j);
+            if (lane == 0) {
+                const uint32_t stage = (cnt0 + j) % STAGES;
+                const uint8_t* src = head_base + (size_t)id * blk_stride;
+                uint8_t* dst = ring + (size_t)stage * 2 * TB;
+                mbar_expect_tx(&bars[stage], 2 * TB);
+                bulk_g2s(dst, src, TB, &bars[stage]);
+                bulk_g2s(dst + TB, src + kv_stride, TB, &bars[stage]);
+            }
+        }
+
+        for (int i = 0; i < nblk; ++i) {
+            const uint32_t stage = cnt % STAGES, parity = (cnt / STAGES) & 1u;
+            mbar_wait(&bars[stage], parity);
+            const uint32_t kt = ring_u32 + stage * 2 * TB, vt = kt + TB;
+            const int nvalid = kv_len - (blk_begin + i) * 16;   // >= 1; < 16 only in the conversation's last block
+            if (nvalid < 16) {
+                // slots past kv_len may hold anything (NaN patterns): 0 * NaN must not reach the PV accumulators
+                uint8_t* vtile = ring + (size_t)stage * 2 * TB + TB;
+                for (int c = lane; c < TB / 16; c += 32)
+                    if (((c & 127) >> 3) >= nvalid) *reinterpret_cast<uint4*>(vtile + c * 16) = make_uint4(0, 0, 0, 0);
+                fence_proxy_async();   // these generic writes precede the next bulk copy into this stage
+                __syncwarp();
+            }
+            // S = Q K^T : 16 (G real) rows x 16 tokens
+            float s0[2] = {0.f, 0.f}, s1[2] = {0.f, 0.f};
+#pragma unroll
+            for (int ks = 0; ks < KS; ++ks) {
+                uint32_t b[4];
+                ldsm_x4(b, kt + (ks >> 2) * 2048 + (k_lane_off ^ (((2 * ks) & 7) << 4)));
+                mma_bf16_top(s0, qa[ks][0], qa[ks][1], b[0], b[1]);
+                mma_bf16_top(s1, qa[ks][0], qa[ks][1], b[2], b[3]);
+            }
+            // scale to the log2 domain, mask by index
+            float sv[4] = {s0[0] * p.scale_log2, s0[1] * p.scale_log2, s1[0] * p.scale_log2, s1[1] * p.scale_log2};
+            if (nvalid < 16) {
+                const int c = 2 * t4;
+                if (c >= nvalid) sv[0] = -INFINITY;
+                if (c + 1 >= nvalid) sv[1] = -INFINITY;
+                if (c + 8 >= nvalid) sv[2] = -INFINITY;
+                if (c + 9 >= nvalid) sv[3] = -INFINITY;
+            }
+            float mx = fmaxf(fmaxf(sv[0], sv[1]), fmaxf(sv[2], sv[3]));
+            mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 1));
+            mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 2));
+            const float m_new = fmaxf(m_run, mx);   // finite: slot 0 of every block is valid
+            if (__any_sync(0xffffffffu, m_new > m_run)) {
+                const float alpha = fast_exp2(m_run - m_new);   // exp2(-inf) = 0 on the first block
+                l_run *= alpha;
+#pragma unroll
+                for (int n = 0; n < NT; ++n) {
+                    o[n][0] *= alpha;
+                    o[n][1] *= alpha;
+                }
+                m_run = m_new;
+            }
+            const float p0 = fast_exp2(sv[0] - m_run), p1 = fast_exp2(sv[1] - m_run);
+            const float p2 = fast_exp2(sv[2] - m_run), p3 = fast_exp2(sv[3] - m_run);
+            l_run += (p0 + p1) + (p2 + p3);
+            const uint32_t pa0 = pack_bf16(p0, p1), pa2 = pack_bf16(p2, p3);
+            // O += P V
+#pragma unroll
+            for (int n2 = 0; n2 < NT / 2; ++n2) {
+                uint32_t b[4];
+                ldsm_x4_trans(b, vt + (n2 >> 2) * 2048 + (v_lane_off ^ (((2 * n2) & 7) << 4)));
+                mma_bf16_top(o[2 * n2], pa0, pa2, b[0], b[1]);
+                mma_bf16_top(o[2 * n2 + 1], pa0, pa2, b[2], b[3]);
+            }
+            __syncwarp();   // every lane is done reading this stage
+            ++cnt;
+            const int nxt = i + STAGES;
+            if (nxt < nblk) {
+                const int id = (nxt >> 5) == grp_cur ? __shfl_sync(0xffffffffu, ids_cur, nxt & 31)
+                                                     : __shfl_sync(0xffffffffu, ids_nxt, nxt & 31);
+                if (lane == 0) {
+                    const uint8_t* src = head_base + (size_t)id * blk_stride;
+                    uint8_t* dst = ring + (size_t)stage * 2 * TB;
+                    mbar_expect_tx(&bars[stage], 2 * TB);
+                    bulk_g2s(dst, src, TB, &bars[stage]);
+                    bulk_g2s(dst + TB, src + kv_stride, TB, &bars[stage]);
+                }
+            }
+            if (((i + 1) & 31) == 0) {
+                ids_cur = ids_nxt;
+                ++grp_cur;
+                const int e = (grp_cur + 1) * 32 + lane;
+                ids_nxt = e < nblk ? __ldg(tab + e) : 0;
+            }
+        }
+
+        // epilogue
+        l_run += __shfl_xor_sync(0xffffffffu, l_run, 1);
+        l_run += __shfl_xor_sync(0xffffffffu, l_run, 2);
+        if (row < G) {
+            if (direct) {
+                const float inv = 1.f / l_run;
+                uint16_t* orow = p.out + ((size_t)conv * p.Hq + (size_t)head * G + row) * D;
+#pragma unroll
+                for (int n = 0; n < NT; ++n)
+                    *reinterpret_cast<uint32_t*>(orow + n * 8 + 2 * t4) = pack_bf16(o[n][0] * inv, o[n][1] * inv);
+                if (t4 == 0) p.lse[(size_t)conv * p.Hq + (size_t)head * G + row] = (m_run + log2f(l_run)) * 0.6931471805599453f;
+            } else {
+                float* orow = p.po + ((size_t)partial * G + row) * D;
+#pragma unroll
+                for (int n = 0; n < NT; ++n) *reinterpret_cast<float2*>(orow + n * 8 + 2 * t4) = make_float2(o[n][0], o[n][1]);
+                if (t4 == 0) *reinterpret_cast<float2*>(p.pml + ((size_t)partial * G + row) * 2) = make_float2(m_run, l_run);
+            }
+        }
+    }
+}
+
+// One warp per (merge group, query head of the group).  Fixed order => deterministic.
+template <int D>
+__global__ void __launch_bounds__(128) decode_merge_kernel(const MergeGroup* groups, int n_groups, int G, int Hq,
+                                                           const float* po, const float* pml, uint16_t* out,
+                                                           float* lse) {
+    constexpr int VEC = D / 32;
+    const int w = blockIdx.x * 4 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (w >= n_groups * G) return;
+    const MergeGroup g = groups[w / G];
+    const int hh = w % G;
+    float M = -INFINITY;
+    for (int k = 0; k < g.count; ++k) M = fmaxf(M, __ldg(pml + ((size_t)(g.first + k) * G + hh) * 2));
+    float L = 0.f, acc[VEC];
+#pragma unroll
+    for (int v = 0; v < VEC; ++v) acc[v] = 0.f;
+    for (int k = 0; k < g.count; ++k) {
+        const float2 ml = __ldg(reinterpret_cast<const float2*>(pml + ((size_t)(g.first + k) * G + hh) * 2));
+        const float wgt = fast_exp2(ml.x - M);
+        L += ml.y * wgt;
+        const float* src = po + ((size_t)(g.first + k) * G + hh) * D + lane * VEC;
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) acc[v] += __ldg(src + v) * wgt;
+    }
+    const float inv = 1.f / L;
+    uint16_t* orow = out + ((size_t)g.conv * Hq + (size_t)g.head * G + hh) * D + lane * VEC;
+#pragma unroll
+    for (int v = 0; v < VEC; v += 2) *reinterpret_cast<uint32_t*>(orow + v) = pack_bf16(acc[v] * inv, acc[v + 1] * inv);
+    if (lane == 0) lse[(size_t)g.conv * Hq + (size_t)g.head * G + hh] = (M + log2f(L)) * 0.6931471805599453f;
+}
+
+template <int D, int STAGES>
+int launch_decode_t(const csv_plan* plan, const DecodeParams& p, cudaStream_t stream) {
+    constexpr int TB = 16 * D * 2;
+    const size_t smem = (size_t)kDecodeWarps * STAGES * 2 * TB + (size_t)kDecodeWarps * STAGES * 8;
+    static bool attr_set = false;
+    if (!attr_set) {
+        CSV_CUDA_TRY(cudaFuncSetAttribute(decode_kernel<D, STAGES>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_set = true;
+    }
+    decode_kernel<D, STAGES><<<plan->decode_grid, kDecodeWarps * 32, smem, stream>>>(p);
+    CSV_CUDA_TRY(cudaGetLastError());
+    const int ng = (int)plan->decode_groups.size();
+    if (ng > 0) {
+        const int warps = ng * p.G;
+        decode_merge_kernel<D><<<(warps + 3) / 4, 128, 0, stream>>>(
+            reinterpret_cast<const MergeGroup*>(plan->d_ws + plan->lay.decode_groups), ng, p.G, p.Hq, p.po, p.pml, p.out,
+            p.lse);
+        CSV_CUDA_TRY(cudaGetLastError());
+    }
+    return CSV_OK;
+}
+
+}   // namespace
+
+int launch_decode(const csv_plan* plan, const kv_pool* pool, int layer, const void* q, const int32_t* tables,
+                  int max_blocks, void* out, float* lse, void* stream) {
+    if (plan->decode_items.empty()) return CSV_OK;
+    const kv_pool_desc& s = pool->desc;
+    DecodeParams p;
+    p.items = reinterpret_cast<const DecodeItem*>(plan->d_ws + plan->lay.decode_items);
+    p.worker_begin = reinterpret_cast<const int32_t*>(plan->d_ws + plan->lay.worker_begin);
+    p.pool_layer = pool->d_base + (size_t)layer * s.num_blocks * 2 * s.num_kv_heads * csv_tile_bytes(s.head_dim);
+    p.q = (const uint16_t*)q;
+    p.tables = tables;
+    p.out = (uint16_t*)out;
+    p.lse = lse;
+    p.po = reinterpret_cast<float*>(plan->d_ws + plan->lay.decode_po);
+    p.pml = reinterpret_cast<float*>(plan->d_ws + plan->lay.decode_pml);
+    p.max_blocks = max_blocks;
+    p.Hq = plan->shape.num_q_heads;
+    p.Hkv = plan->shape.num_kv_heads;
+    p.G = p.Hq / p.Hkv;
+    p.scale_log2 = (float)(1.4426950408889634 / sqrt((double)s.head_dim));
+    if (s.head_dim == 128) return launch_decode_t<128, 3>(plan, p, (cudaStream_t)stream);
+    return launch_decode_t<64, 6>(plan, p, (cudaStream_t)stream);
+}

@@ -1,0 +1,283 @@
+// handoff.cu — kv_pack / kv_unpack / kv_append_tokens: the one-shot KV handoff (a2, a3;
+// PAPER.md:150 §4 "transferred once", §3.1 cost linear in tokens) and the
+// tail step's new-token KV write (§2.1 "appending one new entry").
+//
+// Pure 16-byte moves (bit-exact for any pattern).  Roofline: HBM, read + write bytes.
+//  - pack:   one unit = (conversation, layer, message block, K|V): 16 token rows of
+//            Hkv*d*2 bytes, contiguous in the source (32 KiB at the 8B shape), rewritten as
+//            Hkv tiles in the pool's in-tile format (also 32 KiB contiguous).  Thread ->
+//            consecutive 16-byte source chunks (fully coalesced reads); writes land as
+//            whole 128-byte tile rows.
+//  - unpack: one unit = (conversation, layer, message block): 2*Hkv tiles, contiguous in the
+//            message AND in the pool (64 KiB at the 8B shape): a straight copy to the
+//            block's address from the block table, masked by slot in the first / last block.
+#include "common.cuh"
+#include "internal.h"
+
+namespace {
+
+constexpr int kMaxBatch = 32;        // conversations per launch (descriptors travel as kernel params)
+constexpr int kThreads = 256;
+
+struct PackEntry {
+    const uint8_t* k;
+    const uint8_t* v;
+    uint8_t* staging;
+    int32_t tokens, slot0, ntb, unit_begin;   // units of this entry: [unit_begin, next.unit_begin)
+};
+struct PackParams {
+    PackEntry e[kMaxBatch];
+    int32_t n, total_units, NL, Hkv;
+};
+
+struct UnpackEntry {
+    const uint8_t* staging;
+    const int32_t* ids;     // conversation's table, device
+    int32_t tokens, slot0, ntb, blk0, unit_begin, pad;
+};
+struct UnpackParams {
+    UnpackEntry e[kMaxBatch];
+    int32_t n, total_units, NL, Hkv;
+    int32_t num_blocks, pad;
+    uint8_t* pool;
+};
+
+template <typename P>
+__device__ __forceinline__ int find_entry(const P& p, int unit) {
+    int lo = 0;
+#pragma unroll 1
+    for (int i = 1; i < p.n; ++i)
+        if (p.e[i].unit_begin <= unit) lo = i;
+    return lo;
+}
+
+// D = head_dim.  Chunks (16 B) per token row of one head: D/8.
+template <int D>
+__global__ void __launch_bounds__(kThreads) pack_kernel(const __grid_constant__ PackParams p) {
+    constexpr int CPR = D / 8;                  // chunks per (token, head) row
+    constexpr int TB = 16 * D * 2;              // tile bytes
+    const int chunks_per_unit = 16 * p.Hkv * CPR;   // one (layer, tb, kv): 16 slots x Hkv heads x CPR
+    for (int unit = blockIdx.x; unit < p.total_units; unit += gridDim.x) {
+        const int ei = find_entry(p, unit);
+        const PackEntry& e = p.e[ei];
+        const int u = unit - e.unit_begin;      // ((layer * ntb) + tb) * 2 + kv
+        const int kv = u & 1;
+        const int tb = (u >> 1) % e.ntb;
+        const int layer = (u >> 1) / e.ntb;
+        const uint8_t* src = kv ? e.v : e.k;
+        const size_t row_bytes = (size_t)p.Hkv * D * 2;
+        const uint8_t* src_layer = src + (size_t)layer * e.tokens * row_bytes;
+        uint8_t* dst_unit = e.staging + ((size_t)(layer * e.ntb + tb) * 2 + kv) * p.Hkv * TB;
+        const int tok_base = tb * 16 - e.slot0;   // message token of slot 0 of this block
+        for (int c0 = threadIdx.x; c0 < chunks_per_unit; c0 += kThreads * 4) {
+            uint4 val[4];
+            int dsto[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int c = c0 + j * kThreads;
+                dsto[j] = -1;
+                val[j] = make_uint4(0, 0, 0, 0);
+                if (c < chunks_per_unit) {
+                    const int chunk = c % CPR;
+                    const int head = (c / CPR) % p.Hkv;
+                    const int slot = c / (CPR * p.Hkv);
+                    const int tok = tok_base + slot;
+                    dsto[j] = head * TB + (chunk >> 3) * 2048 + slot * 128 + (((chunk & 7) ^ (slot & 7)) << 4);
+                    if (tok >= 0 && tok < e.tokens)
+                        val[j] = ld_stream(src_layer + (size_t)tok * row_bytes + (size_t)head * D * 2 + chunk * 16);
+                }
+            }
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+                if (dsto[j] >= 0) st_stream(dst_unit + dsto[j], val[j]);
+        }
+    }
+}
+
+template <int D>
+__global__ void __launch_bounds__(kThreads) unpack_kernel(const __grid_constant__ UnpackParams p) {
+    constexpr int TB = 16 * D * 2;
+    constexpr int CPT = TB / 16;                       // chunks per tile
+    const int chunks_per_unit = 2 * p.Hkv * CPT;       // one (layer, tb): K and V tiles of all heads
+    for (int unit = blockIdx.x; unit < p.total_units; unit += gridDim.x) {
+        const int ei = find_entry(p, unit);
+        const UnpackEntry& e = p.e[ei];
+        const int u = unit - e.unit_begin;             // layer * ntb + tb
+        const int tb = u % e.ntb;
+        const int layer = u / e.ntb;
+        const int block = __ldg(e.ids + e.blk0 + tb);
+        const int lo = tb == 0 ? e.slot0 : 0;
+        const int hi = tb == e.ntb - 1 ? ((e.slot0 + e.tokens - 1) & 15) + 1 : 16;
+        const uint8_t* src = e.staging + (size_t)u * chunks_per_unit * 16;
+        uint8_t* dst = p.pool + ((size_t)layer * p.num_blocks + block) * chunks_per_unit * 16;
+        const bool full = lo == 0 && hi == 16;
+        for (int c0 = threadIdx.x; c0 < chunks_per_unit; c0 += kThreads * 4) {
+            uint4 val[4];
+            bool ok[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int c = c0 + j * kThreads;
+                ok[j] = c < chunks_per_unit;
+                if (ok[j] && !full) {
+                    const int slot = ((c % CPT) & 127) >> 3;
+                    ok[j] = slot >= lo && slot < hi;
+                }
+                if (ok[j]) val[j] = ld_stream(src + (size_t)c * 16);
+            }
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+                if (ok[j]) st_stream(dst + (size_t)(c0 + j * kThreads) * 16, val[j]);
+        }
+    }
+}
+
+// New-token KV of a whole batch, token-major [NL][total_q][Hkv][D] -> pool.
+// meta: [q_start[batch+1] | kv_len[batch] | q_len[batch]] on the device.
+template <int D>
+__global__ void __launch_bounds__(kThreads) append_tokens_kernel(uint8_t* pool, int num_blocks, int NL, int Hkv,
+                                                                 const uint8_t* k_new, const uint8_t* v_new,
+                                                                 const int32_t* meta, int batch, int total_q,
+                                                                 const int32_t* tables, int max_blocks) {
+    constexpr int CPR = D / 8;
+    constexpr int TB = 16 * D * 2;
+    const int32_t* q_start = meta;
+    const int32_t* kv_len = meta + batch + 1;
+    const int32_t* q_len = kv_len + batch;
+    const long long total = (long long)NL * total_q * 2 * Hkv * CPR;
+    for (long long idx = (long long)blockIdx.x * kThreads + threadIdx.x; idx < total;
+         idx += (long long)gridDim.x * kThreads) {
+        const int chunk = (int)(idx % CPR);
+        long long r = idx / CPR;
+        const int head = (int)(r % Hkv);
+        r /= Hkv;
+        const int kv = (int)(r & 1);
+        r >>= 1;
+        const int row = (int)(r % total_q);
+        const int layer = (int)(r / total_q);
+        int lo = 0, hi = batch;   // find conv with q_start[conv] <= row < q_start[conv+1]
+        while (hi - lo > 1) {
+            const int mid = (lo + hi) >> 1;
+            if (q_start[mid] <= row) lo = mid; else hi = mid;
+        }
+        const int pos = kv_len[lo] - q_len[lo] + (row - q_start[lo]);
+        const int block = __ldg(tables + (size_t)lo * max_blocks + (pos >> 4));
+        const int slot = pos & 15;
+        const uint8_t* src = (kv ? v_new : k_new) + (((size_t)layer * total_q + row) * Hkv + head) * D * 2 + chunk * 16;
+        uint8_t* dst = pool + ((((size_t)layer * num_blocks + block) * 2 + kv) * Hkv + head) * TB + (chunk >> 3) * 2048 +
+                       slot * 128 + (((chunk & 7) ^ (slot & 7)) << 4);
+        st_stream(dst, ld_stream(src));
+    }
+}
+
+}   // namespace
+
+static int grid_for(int total_units) {
+    const int cap = csv_query_num_sms() * 8;
+    return total_units < cap ? (total_units > 0 ? total_units : 1) : cap;
+}
+
+int launch_pack(const kv_pool_desc& shape, int n, const void* const* k, const void* const* v, const int32_t* tokens,
+                const int32_t* offs, void* const* staging, void* stream) {
+    int i = 0;
+    while (i < n) {
+        PackParams p;
+        p.n = 0;
+        p.NL = shape.num_layers;
+        p.Hkv = shape.num_kv_heads;
+        long long units = 0;
+        while (i < n && p.n < kMaxBatch) {
+            if (tokens[i] > 0) {
+                PackEntry& e = p.e[p.n];
+                e.k = (const uint8_t*)k[i];
+                e.v = (const uint8_t*)v[i];
+                e.staging = (uint8_t*)staging[i];
+                e.tokens = tokens[i];
+                e.slot0 = offs[i] & 15;
+                e.ntb = (e.slot0 + e.tokens + 15) / 16;
+                const long long nu = (long long)shape.num_layers * e.ntb * 2;
+                if (units + nu > INT32_MAX) break;
+                e.unit_begin = (int32_t)units;
+                units += nu;
+                ++p.n;
+            }
+            ++i;
+        }
+        if (p.n == 0) {
+            if (i < n && tokens[i] > 0) return CSV_E_INVAL;   // a single entry too large for one launch
+            continue;
+        }
+        p.total_units = (int32_t)units;
+        const int grid = grid_for(p.total_units);
+        if (shape.head_dim == 128)
+            pack_kernel<128><<<grid, kThreads, 0, (cudaStream_t)stream>>>(p);
+        else
+            pack_kernel<64><<<grid, kThreads, 0, (cudaStream_t)stream>>>(p);
+        CSV_CUDA_TRY(cudaGetLastError());
+    }
+    return CSV_OK;
+}
+
+int launch_unpack(kv_pool* dst, int n, const void* const* staging, const int32_t* tokens, const int32_t* offs,
+                  const int32_t* const* block_ids, void* stream) {
+    const kv_pool_desc& shape = dst->desc;
+    int i = 0;
+    while (i < n) {
+        UnpackParams p;
+        p.n = 0;
+        p.NL = shape.num_layers;
+        p.Hkv = shape.num_kv_heads;
+        p.num_blocks = shape.num_blocks;
+        p.pool = dst->d_base;
+        long long units = 0;
+        while (i < n && p.n < kMaxBatch) {
+            if (tokens[i] > 0) {
+                UnpackEntry& e = p.e[p.n];
+                e.staging = (const uint8_t*)staging[i];
+                e.ids = block_ids[i];
+                e.tokens = tokens[i];
+                e.slot0 = offs[i] & 15;
+                e.ntb = (e.slot0 + e.tokens + 15) / 16;
+                e.blk0 = offs[i] >> 4;
+                const long long nu = (long long)shape.num_layers * e.ntb;
+                if (units + nu > INT32_MAX) break;
+                e.unit_begin = (int32_t)units;
+                units += nu;
+                ++p.n;
+            }
+            ++i;
+        }
+        if (p.n == 0) {
+            if (i < n && tokens[i] > 0) return CSV_E_INVAL;
+            continue;
+        }
+        p.total_units = (int32_t)units;
+        const int grid = grid_for(p.total_units);
+        if (shape.head_dim == 128)
+            unpack_kernel<128><<<grid, kThreads, 0, (cudaStream_t)stream>>>(p);
+        else
+            unpack_kernel<64><<<grid, kThreads, 0, (cudaStream_t)stream>>>(p);
+        CSV_CUDA_TRY(cudaGetLastError());
+    }
+    return CSV_OK;
+}
+
+int launch_append_tokens(kv_pool* dst, const csv_plan* plan, const void* k_new, const void* v_new,
+                         const int32_t* tables, int max_blocks, void* stream) {
+    const kv_pool_desc& s = dst->desc;
+    if (plan->total_q == 0) return CSV_OK;
+    const long long total = (long long)s.num_layers * plan->total_q * 2 * s.num_kv_heads * (s.head_dim / 8);
+    long long blocks = (total + kThreads - 1) / kThreads;
+    const int cap = csv_query_num_sms() * 8;
+    const int grid = (int)(blocks < cap ? blocks : cap);
+    const int32_t* meta = (const int32_t*)(plan->d_ws + plan->lay.conv_meta);
+    if (s.head_dim == 128)
+        append_tokens_kernel<128><<<grid, kThreads, 0, (cudaStream_t)stream>>>(
+            dst->d_base, s.num_blocks, s.num_layers, s.num_kv_heads, (const uint8_t*)k_new, (const uint8_t*)v_new, meta,
+            plan->batch, plan->total_q, tables, max_blocks);
+    else
+        append_tokens_kernel<64><<<grid, kThreads, 0, (cudaStream_t)stream>>>(
+            dst->d_base, s.num_blocks, s.num_layers, s.num_kv_heads, (const uint8_t*)k_new, (const uint8_t*)v_new, meta,
+            plan->batch, plan->total_q, tables, max_blocks);
+    CSV_CUDA_TRY(cudaGetLastError());
+    return CSV_OK;
+}

@@ -1,0 +1,304 @@
+// plan.cpp — host-side step planner: split-K work lists for paged_decode_attn and
+// append_prefill_attn.  Pure host arithmetic on the lengths; the only CUDA call is the
+// asynchronous copy of the finished lists into the caller's workspace (in api.cpp).
+//
+// Decode (SURVEY §7 hard part 4, BASELINE.json config 5 "split-K across >= 64 partitions"):
+// the (conversation, KV head, block) stream of all q_len = 1 rows is flattened in that order
+// and cut into one contiguous share per WARP-worker (decode_grid CTAs x kDecodeWarps warps),
+// so every worker streams the same number of 8 KiB (K tile + V tile) units whatever the
+// length mix.  A share is cut further at (conversation, head) boundaries and every
+// max_partition_tokens tokens.  Each piece is one DecodeItem = one partial (o, m, l).
+// The schedule depends only on the lengths: results are bit-identical under any block
+// permutation and from run to run.
+#include <algorithm>
+#include <new>
+
+#include "internal.h"
+
+static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+static bool attn_shape_ok(const csv_attn_shape* s) {
+    if (!s) return false;
+    if (s->block_size != CSV_BLOCK_SIZE) return false;
+    if (s->head_dim != 64 && s->head_dim != 128) return false;
+    const int hk = s->num_kv_heads;
+    if (hk != 1 && hk != 2 && hk != 4 && hk != 8) return false;
+    if (s->num_q_heads < hk || s->num_q_heads % hk != 0) return false;
+    const int g = s->num_q_heads / hk;
+    if (g != 1 && g != 2 && g != 4 && g != 8) return false;
+    return true;
+}
+
+static void plan_decode(csv_plan* p) {
+    const int Hkv = p->shape.num_kv_heads;
+    const int part_blocks = std::max(1, p->max_partition_tokens / CSV_BLOCK_SIZE);
+    int64_t units = 0;
+    p->n_decode_rows = 0;
+    for (int b = 0; b < p->batch; ++b)
+        if (p->q_lens[b] == 1) {
+            units += (int64_t)((p->kv_lens[b] + CSV_BLOCK_SIZE - 1) / CSV_BLOCK_SIZE) * Hkv;
+            ++p->n_decode_rows;
+        }
+    // CTAs: one per SM, fewer when there is under 4 blocks of work per warp
+    int64_t want = (units + (int64_t)kDecodeWarps * 4 - 1) / ((int64_t)kDecodeWarps * 4);
+    p->decode_grid = (int)std::max<int64_t>(1, std::min<int64_t>(p->num_sms, want));
+    const int64_t W = (int64_t)p->decode_grid * kDecodeWarps;
+    p->worker_begin.assign((size_t)W + 1, 0);
+    p->decode_items.clear();
+    p->decode_groups.clear();
+    p->n_decode_partials = 0;
+    if (units == 0) return;
+
+    int64_t base = 0;   // first unit of the current (conv, head) segment
+    int64_t w = 0;      // worker whose share contains `pos`
+    auto share_start = [&](int64_t k) { return (k * units) / W; };
+    for (int b = 0; b < p->batch; ++b) {
+        if (p->q_lens[b] != 1) continue;
+        const int nblk = (p->kv_lens[b] + CSV_BLOCK_SIZE - 1) / CSV_BLOCK_SIZE;
+        for (int g = 0; g < Hkv; ++g) {
+            const size_t first_item = p->decode_items.size();
+            int blk = 0;
+            while (blk < nblk) {
+                const int64_t pos = base + blk;
+                while (w + 1 < W && share_start(w + 1) <= pos) {   // advance to the worker owning pos
+                    ++w;
+                    p->worker_begin[(size_t)w] = (int32_t)p->decode_items.size();
+                }
+                const int64_t share_end = share_start(w + 1);   // == units for the last worker
+                int end = (int)std::min<int64_t>(nblk, share_end - base);
+                end = std::min(end, blk + part_blocks);
+                DecodeItem it{};
+                it.conv = b;
+                it.head = g;
+                it.blk_begin = blk;
+                it.blk_end = end;
+                it.kv_len = p->kv_lens[b];
+                it.partial = -1;
+                it.direct = 0;
+                p->decode_items.push_back(it);
+                blk = end;
+            }
+            const size_t n = p->decode_items.size() - first_item;
+            if (n == 1) {
+                p->decode_items[first_item].direct = 1;
+            } else {
+                MergeGroup mg{};
+                mg.first = p->n_decode_partials;
+                mg.count = (int32_t)n;
+                mg.conv = b;
+                mg.head = g;
+                for (size_t i = 0; i < n; ++i) p->decode_items[first_item + i].partial = p->n_decode_partials++;
+                p->decode_groups.push_back(mg);
+            }
+            base += nblk;
+        }
+    }
+    for (int64_t k = w + 1; k <= W; ++k) p->worker_begin[(size_t)k] = (int32_t)p->decode_items.size();
+}
+
+static void plan_append(csv_plan* p) {
+    const int Hkv = p->shape.num_kv_heads;
+    const int G = p->shape.num_q_heads / Hkv;
+    p->n_append_chunks = 0;
+    p->n_append_rows = 0;
+    p->append_items.clear();
+    p->append_groups.clear();
+    p->n_append_partials = 0;
+    for (int b = 0; b < p->batch; ++b)
+        if (p->q_lens[b] > 1) {
+            ++p->n_append_chunks;
+            p->n_append_rows += p->q_lens[b];
+        }
+    if (p->n_append_chunks == 0) return;
+
+    auto count_items = [&](int split_blocks) {
+        int64_t n = 0;
+        for (int b = 0; b < p->batch; ++b) {
+            const int m = p->q_lens[b];
+            if (m <= 1) continue;
+            const int P = p->kv_lens[b] - m;
+            const int rows = m * G;
+            for (int r0 = 0; r0 < rows; r0 += kAppendTileRows) {
+                const int i_max = std::min(m - 1, (std::min(rows, r0 + kAppendTileRows) - 1) / G);
+                const int nblk = (P + i_max + 1 + CSV_BLOCK_SIZE - 1) / CSV_BLOCK_SIZE;
+                n += (int64_t)Hkv * ((nblk + split_blocks - 1) / split_blocks);
+            }
+        }
+        return n;
+    };
+    int split_blocks;
+    if (p->max_partition_tokens_user > 0) {
+        split_blocks = std::max(1, p->max_partition_tokens_user / CSV_BLOCK_SIZE);
+    } else {
+        // largest power-of-two split (<= 2^17 tokens) that still gives >= 6 items per CTA slot
+        const int64_t slots = (int64_t)p->num_sms * 2;
+        split_blocks = (1 << 17) / CSV_BLOCK_SIZE;
+        while (split_blocks > 2048 / CSV_BLOCK_SIZE && count_items(split_blocks) < 6 * slots) split_blocks /= 2;
+    }
+
+    for (int b = 0; b < p->batch; ++b) {
+        const int m = p->q_lens[b];
+        if (m <= 1) continue;
+        const int P = p->kv_lens[b] - m;
+        const int rows = m * G;
+        for (int g = 0; g < Hkv; ++g)
+            for (int r0 = 0; r0 < rows; r0 += kAppendTileRows) {
+                const int i_max = std::min(m - 1, (std::min(rows, r0 + kAppendTileRows) - 1) / G);
+                const int nblk = (P + i_max + 1 + CSV_BLOCK_SIZE - 1) / CSV_BLOCK_SIZE;
+                const int nparts = (nblk + split_blocks - 1) / split_blocks;
+                MergeGroup mg{};
+                mg.first = p->n_append_partials;
+                mg.count = nparts;
+                mg.conv = b;
+                mg.head = g;
+                mg.row_begin = r0;
+                mg.q_start = p->q_start[b];
+                mg.m = m;
+                for (int k = 0; k < nparts; ++k) {
+                    AppendItem it{};
+                    it.conv = b;
+                    it.head = g;
+                    it.row_begin = r0;
+                    it.q_start = p->q_start[b];
+                    it.m = m;
+                    it.kv_len = p->kv_lens[b];
+                    it.blk_begin = k * split_blocks;
+                    it.blk_end = std::min(nblk, (k + 1) * split_blocks);
+                    it.direct = nparts == 1 ? 1 : 0;
+                    it.partial = nparts == 1 ? -1 : p->n_append_partials++;
+                    p->append_items.push_back(it);
+                }
+                if (nparts > 1) p->append_groups.push_back(mg);
+            }
+    }
+    // longest first (static round-robin over CTAs in the kernel); stable => deterministic
+    std::stable_sort(p->append_items.begin(), p->append_items.end(), [](const AppendItem& a, const AppendItem& b) {
+        return (a.blk_end - a.blk_begin) > (b.blk_end - b.blk_begin);
+    });
+}
+
+static void plan_layout(csv_plan* p) {
+    const int d = p->shape.head_dim;
+    const int G = p->shape.num_q_heads / p->shape.num_kv_heads;
+    PlanLayout& L = p->lay;
+    size_t off = 0;
+    auto take = [&](size_t bytes) {
+        const size_t at = off;
+        off = align_up(off + bytes, 128);
+        return at;
+    };
+    L.decode_items = take(p->decode_items.size() * sizeof(DecodeItem));
+    L.worker_begin = take(p->worker_begin.size() * sizeof(int32_t));
+    L.decode_groups = take(p->decode_groups.size() * sizeof(MergeGroup));
+    L.append_items = take(p->append_items.size() * sizeof(AppendItem));
+    L.append_groups = take(p->append_groups.size() * sizeof(MergeGroup));
+    std::vector<int32_t> meta;
+    meta.insert(meta.end(), p->q_start.begin(), p->q_start.end());
+    meta.insert(meta.end(), p->kv_lens.begin(), p->kv_lens.end());
+    meta.insert(meta.end(), p->q_lens.begin(), p->q_lens.end());
+    L.conv_meta = take(meta.size() * sizeof(int32_t));
+    const size_t list_bytes = off;
+    L.decode_po = take((size_t)p->n_decode_partials * G * d * sizeof(float));
+    L.decode_pml = take((size_t)p->n_decode_partials * G * 2 * sizeof(float));
+    L.append_po = take((size_t)p->n_append_partials * kAppendTileRows * d * sizeof(float));
+    L.append_pml = take((size_t)p->n_append_partials * kAppendTileRows * 2 * sizeof(float));
+    L.total = std::max<size_t>(off, 128);
+    p->h_image.assign(list_bytes, 0);
+    auto put = [&](size_t at, const void* src, size_t bytes) {
+        if (bytes) memcpy(p->h_image.data() + at, src, bytes);
+    };
+    put(L.decode_items, p->decode_items.data(), p->decode_items.size() * sizeof(DecodeItem));
+    put(L.worker_begin, p->worker_begin.data(), p->worker_begin.size() * sizeof(int32_t));
+    put(L.decode_groups, p->decode_groups.data(), p->decode_groups.size() * sizeof(MergeGroup));
+    put(L.append_items, p->append_items.data(), p->append_items.size() * sizeof(AppendItem));
+    put(L.append_groups, p->append_groups.data(), p->append_groups.size() * sizeof(MergeGroup));
+    put(L.conv_meta, meta.data(), meta.size() * sizeof(int32_t));
+}
+
+// Builds the host side of a plan.  Returns NULL on bad arguments.
+csv_plan* csv_plan_build_host(const csv_attn_shape* shape, const int32_t* h_q_lens, const int32_t* h_kv_lens,
+                              int32_t batch, int32_t max_partition_tokens, int* err) {
+    *err = CSV_E_INVAL;
+    if (!attn_shape_ok(shape) || batch < 0 || (batch > 0 && (!h_q_lens || !h_kv_lens))) return nullptr;
+    if (max_partition_tokens < 0 || max_partition_tokens % CSV_BLOCK_SIZE != 0) return nullptr;
+    int64_t total_q = 0;
+    for (int b = 0; b < batch; ++b) {
+        if (h_kv_lens[b] < 0 || h_q_lens[b] < 0 || h_q_lens[b] > h_kv_lens[b]) return nullptr;
+        total_q += h_q_lens[b];
+    }
+    if (total_q > INT32_MAX) return nullptr;
+    csv_plan* p = new (std::nothrow) csv_plan();
+    if (!p) {
+        *err = CSV_E_NOMEM;
+        return nullptr;
+    }
+    p->shape = *shape;
+    p->batch = batch;
+    p->max_partition_tokens_user = max_partition_tokens;
+    p->max_partition_tokens = max_partition_tokens > 0 ? max_partition_tokens : 2048;
+    p->num_sms = csv_query_num_sms();
+    p->q_lens.assign(h_q_lens, h_q_lens + batch);
+    p->kv_lens.assign(h_kv_lens, h_kv_lens + batch);
+    p->q_start.assign((size_t)batch + 1, 0);
+    for (int b = 0; b < batch; ++b) p->q_start[(size_t)b + 1] = p->q_start[(size_t)b] + h_q_lens[b];
+    p->total_q = (int32_t)total_q;
+    p->d_ws = nullptr;
+    plan_decode(p);
+    plan_append(p);
+    plan_layout(p);
+    *err = CSV_OK;
+    return p;
+}
+
+extern "C" {
+
+size_t csv_plan_workspace_bytes(const csv_attn_shape* shape, const int32_t* h_q_lens, const int32_t* h_kv_lens,
+                                int32_t batch, int32_t max_partition_tokens) {
+    int err;
+    csv_plan* p = csv_plan_build_host(shape, h_q_lens, h_kv_lens, batch, max_partition_tokens, &err);
+    if (!p) return 0;
+    const size_t n = p->lay.total;
+    delete p;
+    return n;
+}
+
+int csv_plan_destroy(csv_plan_t* plan) {
+    if (!plan) return CSV_E_INVAL;
+    delete plan;
+    return CSV_OK;
+}
+
+int csv_plan_info(const csv_plan_t* plan, int32_t* n_decode_items, int32_t* n_decode_rows, int32_t* n_append_chunks,
+                  int32_t* n_append_rows, int32_t* decode_grid) {
+    if (!plan) return CSV_E_INVAL;
+    if (n_decode_items) *n_decode_items = (int32_t)plan->decode_items.size();
+    if (n_decode_rows) *n_decode_rows = plan->n_decode_rows;
+    if (n_append_chunks) *n_append_chunks = plan->n_append_chunks;
+    if (n_append_rows) *n_append_rows = plan->n_append_rows;
+    if (decode_grid) *decode_grid = plan->decode_grid;
+    return CSV_OK;
+}
+
+int32_t csv_plan_total_q(const csv_plan_t* plan) { return plan ? plan->total_q : -1; }
+
+int32_t csv_plan_decode_items(const csv_plan_t* plan, int32_t* h_out, int32_t max_items, int32_t* h_worker_begin,
+                              int32_t max_workers_plus_1) {
+    if (!plan) return -1;
+    const int32_t n = (int32_t)plan->decode_items.size();
+    if (h_out)
+        for (int32_t i = 0; i < n && i < max_items; ++i) memcpy(h_out + (size_t)i * 8, &plan->decode_items[(size_t)i], 32);
+    if (h_worker_begin)
+        for (int32_t i = 0; i < (int32_t)plan->worker_begin.size() && i < max_workers_plus_1; ++i)
+            h_worker_begin[i] = plan->worker_begin[(size_t)i];
+    return n;
+}
+
+int32_t csv_plan_append_items(const csv_plan_t* plan, int32_t* h_out, int32_t max_items) {
+    if (!plan) return -1;
+    const int32_t n = (int32_t)plan->append_items.size();
+    if (h_out)
+        for (int32_t i = 0; i < n && i < max_items; ++i) memcpy(h_out + (size_t)i * 12, &plan->append_items[(size_t)i], 48);
+    return n;
+}
+
+}   // extern "C"
