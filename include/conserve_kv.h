@@ -242,7 +242,7 @@ int csv_plan_info(const csv_plan_t* plan, int32_t* n_decode_items, int32_t* n_de
 /* Sum of the plan's q_lens (rows of d_q / d_out for append_prefill_attn); -1 on NULL. */
 int32_t csv_plan_total_q(const csv_plan_t* plan);
 /* Copies the decode work list for inspection (host tests): item i is 8 int32
- * {conv, kv_head, blk_begin, blk_end, kv_len, partial, direct, 0} at h_out[8*i];
+ * {conv, kv_head, blk_begin, blk_end, kv_len, partial, direct, q_row} at h_out[8*i];
  * h_worker_begin[w] .. h_worker_begin[w+1] are the items of warp-worker w
  * (decode_grid * 8 workers).  Either output may be NULL.  Returns the item count. */
 int32_t csv_plan_decode_items(const csv_plan_t* plan, int32_t* h_out, int32_t max_items,
@@ -264,9 +264,11 @@ int32_t csv_plan_append_items(const csv_plan_t* plan, int32_t* h_out, int32_t ma
  * kv_len = 0 -> O = 0, LSE = -inf.  bf16 inputs, fp32 scores / softmax /
  * accumulation; softmax weights are rounded to bf16 for the PV product.
  *
- * d_q:   [batch][Hq][d] bf16 (row b is read only if q_len[b] = 1), 16-byte aligned.
+ * d_q:   [total_q][Hq][d] bf16, 16-byte aligned, total_q = sum of ALL q_lens of the plan in
+ *        batch order (= [batch][Hq][d] when every q_len is 1); conversation b's row is
+ *        sum_{b'<b} q_len[b'] and is read only if q_len[b] = 1.
  * d_block_tables: [batch][max_blocks] int32; entries past ceil(kv_len/16) are never read.
- * d_out: [batch][Hq][d] bf16;  d_lse: [batch][Hq] fp32.  Rows with q_len != 1 are untouched.
+ * d_out: [total_q][Hq][d] bf16;  d_lse: [total_q][Hq] fp32.  Rows with q_len != 1 are untouched.
  * Pool slots past kv_len in the last block may hold anything (NaN patterns included).
  * ---------------------------------------------------------------------- */
 int paged_decode_attn(const csv_plan_t* plan, const kv_pool_t* pool, int32_t layer, const void* d_q,
@@ -282,9 +284,8 @@ int paged_decode_attn(const csv_plan_t* plan, const kv_pool_t* pool, int32_t lay
  * keys 0 .. P + i (prefix fully visible, causal inside the chunk, diagonal
  * included).  Same softmax, outputs and precision as paged_decode_attn.
  *
- * d_q / d_out: [total_q][Hq][d] bf16 with total_q = sum of ALL q_lens of the
- * plan (decode rows included, in batch order; decode rows are skipped here).
- * d_lse: [total_q][Hq] fp32.
+ * d_q / d_out / d_lse: the same [total_q] buffers as paged_decode_attn (decode
+ * rows are skipped here), so one step's two calls fill one output.
  * ---------------------------------------------------------------------- */
 int append_prefill_attn(const csv_plan_t* plan, const kv_pool_t* pool, int32_t layer, const void* d_q,
                         const int32_t* d_block_tables, int32_t max_blocks, void* d_out, float* d_lse,

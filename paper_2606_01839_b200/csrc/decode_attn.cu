@@ -75,7 +75,7 @@ __global__ void __launch_bounds__(kDecodeWarps * 32, 1) decode_kernel(const __gr
         const int4 i0 = __ldg(reinterpret_cast<const int4*>(p.items + ii));
         const int4 i1 = __ldg(reinterpret_cast<const int4*>(p.items + ii) + 1);
         const int conv = i0.x, head = i0.y, blk_begin = i0.z, blk_end = i0.w;
-        const int kv_len = i1.x, partial = i1.y, direct = i1.z;
+        const int kv_len = i1.x, partial = i1.y, direct = i1.z, q_row = i1.w;
         const int nblk = blk_end - blk_begin;
         const int32_t* tab = p.tables + (size_t)conv * p.max_blocks + blk_begin;
         int ids_cur = lane < nblk ? __ldg(tab + lane) : 0;
@@ -85,7 +85,7 @@ __global__ void __launch_bounds__(kDecodeWarps * 32, 1) decode_kernel(const __gr
         // Q fragments: row `row` of the group (zero beyond G); rows 8..15 of the MMA are zero
         uint32_t qa[KS][2];
         {
-            const uint16_t* qrow = p.q + ((size_t)conv * p.Hq + (size_t)head * G + row) * D;
+            const uint16_t* qrow = p.q + ((size_t)q_row * p.Hq + (size_t)head * G + row) * D;
 #pragma unroll
             for (int ks = 0; ks < KS; ++ks) {
                 qa[ks][0] = row < G ? *reinterpret_cast<const uint32_t*>(qrow + ks * 16 + 2 * t4) : 0u;
@@ -198,11 +198,11 @@ __global__ void __launch_bounds__(kDecodeWarps * 32, 1) decode_kernel(const __gr
         if (row < G) {
             if (direct) {
                 const float inv = 1.f / l_run;
-                uint16_t* orow = p.out + ((size_t)conv * p.Hq + (size_t)head * G + row) * D;
+                uint16_t* orow = p.out + ((size_t)q_row * p.Hq + (size_t)head * G + row) * D;
 #pragma unroll
                 for (int n = 0; n < NT; ++n)
                     *reinterpret_cast<uint32_t*>(orow + n * 8 + 2 * t4) = pack_bf16(o[n][0] * inv, o[n][1] * inv);
-                if (t4 == 0) p.lse[(size_t)conv * p.Hq + (size_t)head * G + row] = (m_run + log2f(l_run)) * 0.6931471805599453f;
+                if (t4 == 0) p.lse[(size_t)q_row * p.Hq + (size_t)head * G + row] = (m_run + log2f(l_run)) * 0.6931471805599453f;
             } else {
                 float* orow = p.po + ((size_t)partial * G + row) * D;
 #pragma unroll
@@ -237,10 +237,10 @@ __global__ void __launch_bounds__(128) decode_merge_kernel(const MergeGroup* gro
         for (int v = 0; v < VEC; ++v) acc[v] += __ldg(src + v) * wgt;
     }
     const float inv = 1.f / L;
-    uint16_t* orow = out + ((size_t)g.conv * Hq + (size_t)g.head * G + hh) * D + lane * VEC;
+    uint16_t* orow = out + ((size_t)g.q_start * Hq + (size_t)g.head * G + hh) * D + lane * VEC;
 #pragma unroll
     for (int v = 0; v < VEC; v += 2) *reinterpret_cast<uint32_t*>(orow + v) = pack_bf16(acc[v] * inv, acc[v + 1] * inv);
-    if (lane == 0) lse[(size_t)g.conv * Hq + (size_t)g.head * G + hh] = (M + log2f(L)) * 0.6931471805599453f;
+    if (lane == 0) lse[(size_t)g.q_start * Hq + (size_t)g.head * G + hh] = (M + log2f(L)) * 0.6931471805599453f;
 }
 
 template <int D, int STAGES>

@@ -32,7 +32,7 @@ struct DecodeItem {
     int32_t kv_len;
     int32_t partial;   // index into the decode partial arrays
     int32_t direct;    // 1 = the only partition of its (conv, head): write O / LSE directly
-    int32_t pad;
+    int32_t q_row;     // row of this conversation in d_q / d_out / d_lse (= sum of earlier q_lens)
 };
 
 // One append work item: a tile of stacked rows (token-major: row r = i * G + hh) of one

@@ -75,6 +75,7 @@ static void plan_decode(csv_plan* p) {
                 it.kv_len = p->kv_lens[b];
                 it.partial = -1;
                 it.direct = 0;
+                it.q_row = p->q_start[(size_t)b];
                 p->decode_items.push_back(it);
                 blk = end;
             }
@@ -87,6 +88,7 @@ static void plan_decode(csv_plan* p) {
                 mg.count = (int32_t)n;
                 mg.conv = b;
                 mg.head = g;
+                mg.q_start = p->q_start[(size_t)b];
                 for (size_t i = 0; i < n; ++i) p->decode_items[first_item + i].partial = p->n_decode_partials++;
                 p->decode_groups.push_back(mg);
             }

@@ -1,0 +1,100 @@
+"""GPU parity of append_prefill_attn (and mixed decode + append steps, and the host-buffer tail
+step) against the fp64 oracle.  PAPER.md:94 §3.1: appended chunks attend to "the whole history
+context" plus themselves; BASELINE.json config 3: "causal against prefix+self".
+"""
+import numpy as np
+import pytest
+import torch
+
+from paper_2606_01839_b200 import binding as B
+from paper_2606_01839_b200 import synth
+from harness import Scenario, assert_close, bf16_dev_to_f64, dev, oracle_attention, run_attention, u16_dev
+
+pytestmark = pytest.mark.gpu
+
+
+def step_case(oracle, seed, Hq, Hkv, d, convs, mpt=0, poison=False, v_mean=0.0, qscale=1.0, what=""):
+    """convs: list of (P, m); m = 1 is a decode row (kv_len = P + 1), m = 0 an inert conversation."""
+    rng = np.random.default_rng(seed)
+    q_lens = [m for _, m in convs]
+    kv_lens = [P + m for P, m in convs]
+    sc = Scenario(oracle, rng, Hq, Hkv, d, kv_lens, poison=poison, v_mean=v_mean).commit().upload()
+    q = synth.normal_bf16(rng, (sum(q_lens), Hq, d), std=qscale)
+    O, LSE, info = run_attention(sc, q_lens, q, mpt=mpt, which="both")
+    O_ref, LSE_ref = oracle_attention(sc, q_lens, q)
+    return assert_close(O, LSE, O_ref, LSE_ref, what or "step"), info
+
+
+@pytest.mark.parametrize("Hq,Hkv,d", [(32, 8, 128), (64, 8, 128), (4, 1, 64), (8, 8, 64), (16, 2, 128)])
+def test_append_chunk_length_edge_cases(oracle, Hq, Hkv, d):
+    # m in {2, 31, 32, 33, 512}, P = 0, prefixes not multiples of 16
+    convs = [(0, 2), (0, 33), (100, 31), (1000, 32), (17, 33), (777, 2), (15, 16), (3, 100)]
+    step_case(oracle, 50 + Hq + d, Hq, Hkv, d, convs, what="append edges %s" % ((Hq, Hkv, d),))
+
+
+def test_append_512_token_chunk_and_full_causal_prefill(oracle):
+    step_case(oracle, 60, 32, 8, 128, [(2000, 512), (0, 300)], what="m=512")
+
+
+def test_mixed_decode_and_append_step_fills_one_output(oracle):
+    # one plan, two calls, one [total_q] output: decode rows and chunks interleaved in batch order
+    convs = [(500, 1), (300, 40), (0, 1), (2047, 1), (64, 64), (10, 0), (4000, 1), (129, 17)]
+    step_case(oracle, 61, 32, 8, 128, convs, what="mixed")
+    step_case(oracle, 62, 64, 8, 128, convs, what="mixed G=8")
+
+
+@pytest.mark.parametrize("mpt", [64, 256, 2048])
+def test_append_kv_partitions_merge_correctly(oracle, mpt):
+    # long prefix cut into KV partitions; a partition boundary inside the chunk's own tokens leaves some rows
+    # with no visible key in the last partition (their partial is m = -inf, l = 0)
+    convs = [(3000, 100), (250, 200), (0, 130), (5000, 33)]
+    (_, _), info = step_case(oracle, 63, 32, 8, 128, convs, mpt=mpt, what="append mpt=%d" % mpt)
+
+
+def test_append_poisoned_padding_and_nonzero_mean(oracle):
+    step_case(oracle, 64, 32, 8, 128, [(100, 37), (1000, 5), (3, 2)], poison=True, what="append poison")
+    step_case(oracle, 65, 32, 8, 128, [(3000, 64), (9000, 40)], v_mean=1.0, what="append V~N(1,1)")
+    step_case(oracle, 66, 32, 8, 128, [(2000, 48)], qscale=8.0, what="append q x8")
+
+
+def test_append_row_equals_decode_on_the_truncated_cache(oracle):
+    """Row i of a chunk with prefix P must equal a decode row with kv_len = P + i + 1 on the same cache
+    (the oracle's invariant, now across the two CUDA kernels)."""
+    rng = np.random.default_rng(67)
+    Hq, Hkv, d, P, m = 32, 8, 128, 700, 24
+    sc = Scenario(oracle, rng, Hq, Hkv, d, [P + m]).commit().upload()
+    q = synth.normal_bf16(rng, (m, Hq, d))
+    O_a, LSE_a, _ = run_attention(sc, [m], q, which="append")
+    for i in (0, 7, m - 1):
+        sc.kv_lens = [P + i + 1]
+        O_d, LSE_d, _ = run_attention(sc, [1], q[i:i + 1], which="decode")
+        assert np.abs(O_d[0] - O_a[i]).max() <= 2 ** -7 and np.abs(LSE_d[0] - LSE_a[i]).max() <= 2e-4
+    sc.kv_lens = [P + m]
+
+
+def test_tail_step_host_buffers(oracle):
+    """csv_tail_step_host: plan + H2D + new-token KV write + decode + D2H in one call (bench.py's e2e path)."""
+    rng = np.random.default_rng(68)
+    Hq, Hkv, d = 32, 8, 128
+    kv_lens = [100, 2049, 16, 1, 777]
+    sc = Scenario(oracle, rng, Hq, Hkv, d, kv_lens, poison=True)
+    # the cache holds everything but each conversation's newest token; that token arrives through the call
+    k_new = np.stack([sc.K[b][0, kv_lens[b] - 1] for b in range(5)])
+    v_new = np.stack([sc.V[b][0, kv_lens[b] - 1] for b in range(5)])
+    for b, t in enumerate(kv_lens):
+        if t > 1:
+            sc.image = oracle.scatter(sc.image, 1, sc.num_blocks, Hkv, d, sc.K[b][:, :t - 1], sc.V[b][:, :t - 1], t - 1, 0,
+                                      sc.tables[b])
+    sc.upload()
+    shape = B.attn_shape(Hq, Hkv, d)
+    q = synth.normal_bf16(rng, (5, Hq, d))
+    tabs = np.where(sc.h_tables < 0, 0, sc.h_tables).astype(np.int32)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    h_q, h_k, h_v, h_t = pin(q.view(np.int16)), pin(k_new.view(np.int16)), pin(v_new.view(np.int16)), pin(tabs)
+    h_out = torch.zeros((5, Hq, d), dtype=torch.int16).pin_memory()
+    h_lse = torch.zeros((5, Hq), dtype=torch.float32).pin_memory()
+    ws = torch.empty(B.csv_tail_step_host_workspace_bytes(shape, kv_lens, sc.max_blocks), dtype=torch.uint8, device="cuda")
+    B.csv_tail_step_host(sc.pool, 0, shape, kv_lens, h_q, h_k, h_v, h_t, sc.max_blocks, ws, h_out, h_lse)
+    O = synth.bf16_bits_to_f32(h_out.numpy().view(np.uint16)).astype(np.float64)
+    O_ref, LSE_ref = oracle_attention(sc, [1] * 5, q)
+    assert_close(O, h_lse.numpy().astype(np.float64), O_ref, LSE_ref, what="tail step")

@@ -1,0 +1,135 @@
+"""GPU parity of the one-shot KV handoff (kv_pack / kv_unpack / kv_append_tokens) against the
+oracle's reference scatter (O3) and staging formula.  Bit-exact, whole pool image compared
+(a stray write anywhere is a mismatch).  PAPER.md:150 §4 "transferred once to the bound decoder".
+"""
+import numpy as np
+import pytest
+import torch
+
+from paper_2606_01839_b200 import binding as B
+from paper_2606_01839_b200 import synth
+from harness import dev, dev_to_u16, u16_dev
+
+pytestmark = pytest.mark.gpu
+GUARD = 0xA5C3
+
+
+def handoff_case(oracle, rng, NL, Hkv, d, num_blocks, convs, batched):
+    """convs: list of (tokens, token_offset).  Each conversation owns ceil((off+tokens)/16) blocks."""
+    desc = B.pool_desc(NL, num_blocks, Hkv, d)
+    image = np.full(oracle.pool_elems(NL, num_blocks, Hkv, d), GUARD, dtype=np.uint16)
+    d_image = u16_dev(image)
+    pool = B.KvPool(desc, d_image)
+    pool.set_free_order(synth.shuffled_free_order(rng, num_blocks))
+    expected = image.copy()
+    ks, vs, stagings, tables, toks, offs, nids, msgs = [], [], [], [], [], [], [], []
+    for tokens, off in convs:
+        ids = pool.alloc_blocks(synth.blocks_for(off + tokens))
+        K = synth.random_bits(rng, (NL, tokens, Hkv, d))
+        V = synth.random_bits(rng, (NL, tokens, Hkv, d))
+        expected = oracle.scatter(expected, NL, num_blocks, Hkv, d, K, V, tokens, off, ids)
+        msgs.append(oracle.staging_message(NL, Hkv, d, K, V, tokens, off))
+        nbytes = B.kv_staging_bytes(desc, tokens, off)
+        assert nbytes == msgs[-1].size * 2
+        ks.append(u16_dev(K))
+        vs.append(u16_dev(V))
+        stagings.append(torch.full((nbytes // 2,), 0x1111, dtype=torch.int16, device="cuda"))
+        tables.append(dev(ids))
+        toks.append(tokens)
+        offs.append(off)
+        nids.append(len(ids))
+    if batched:
+        B.kv_pack_batch(desc, ks, vs, toks, offs, stagings)
+        B.kv_unpack_batch(pool, stagings, toks, offs, tables, nids)
+    else:
+        for i in range(len(convs)):
+            B.kv_pack(desc, ks[i], vs[i], toks[i], offs[i], stagings[i])
+            B.kv_unpack(pool, stagings[i], toks[i], offs[i], tables[i], nids[i])
+    torch.cuda.synchronize()
+    for i in range(len(convs)):
+        assert np.array_equal(dev_to_u16(stagings[i]), msgs[i]), "staging message %d differs from the oracle's" % i
+    got = dev_to_u16(d_image)
+    assert np.array_equal(got, expected), "pool image differs (%d elements)" % int((got != expected).sum())
+    return pool
+
+
+def test_config1_handoff_300_tokens(oracle):
+    # BASELINE.json config 1: one kv_pack / kv_unpack of a 300-token prefill into a second 256-block pool
+    rng = np.random.default_rng(0)
+    pool = handoff_case(oracle, rng, 1, 1, 64, 256, [(300, 0)], batched=False)
+    assert pool.used_blocks == 19
+
+
+@pytest.mark.parametrize("batched", [False, True])
+def test_handoff_8b_shape_ragged_and_offsets(oracle, batched):
+    rng = np.random.default_rng(7)
+    convs = [(300, 0), (1, 0), (16, 0), (17, 0), (5, 11), (1, 15), (2, 15), (40, 24), (129, 3), (33, 32)]
+    handoff_case(oracle, rng, 3, 8, 128, 64, convs, batched)
+
+
+def test_handoff_other_shapes(oracle):
+    rng = np.random.default_rng(8)
+    handoff_case(oracle, rng, 2, 2, 64, 40, [(100, 0), (7, 9), (64, 16)], batched=True)
+    handoff_case(oracle, rng, 1, 4, 128, 40, [(47, 0), (20, 5)], batched=True)
+
+
+def test_handoff_more_conversations_than_one_launch_holds(oracle):
+    rng = np.random.default_rng(9)
+    convs = [(int(rng.integers(1, 40)), int(rng.integers(0, 16))) for _ in range(70)]
+    handoff_case(oracle, rng, 1, 2, 64, 4 * 70 + 5, convs, batched=True)
+
+
+def test_handoff_argument_errors():
+    desc = B.pool_desc(1, 8, 1, 64)
+    buf = torch.zeros(B.kv_pool_bytes(desc) // 2, dtype=torch.int16, device="cuda")
+    pool = B.KvPool(desc, buf)
+    k = torch.zeros(300 * 64, dtype=torch.int16, device="cuda")
+    st = torch.zeros(B.kv_staging_bytes(desc, 300) // 2, dtype=torch.int16, device="cuda")
+    ids = torch.zeros(8, dtype=torch.int32, device="cuda")
+    before = buf.clone()
+    for call in (lambda: B.kv_pack(desc, k, k, 0, 0, st),                       # zero tokens
+                 lambda: B.kv_pack(desc, k, k, -1, 0, st),
+                 lambda: B.kv_pack(desc, k, k, 10, -1, st),
+                 lambda: B.kv_pack(desc, k, k, 10, 0, st.data_ptr() + 16),      # misaligned staging
+                 lambda: B.kv_pack(desc, k.data_ptr() + 2, k, 10, 0, st),       # misaligned source
+                 lambda: B.kv_pack(B.pool_desc(1, 8, 3, 64), k, k, 10, 0, st),  # unsupported shape
+                 lambda: B.kv_unpack(pool, st, 300, 0, ids, 8),                 # table shorter than ceil(300/16)
+                 lambda: B.kv_unpack(pool, st, 17, 112, ids, 8),                # offset + tokens past the table
+                 lambda: B.kv_unpack(pool, st, 0, 0, ids, 8)):
+        with pytest.raises(B.CsvError) as e:
+            call()
+        assert e.value.code == B.CSV_E_INVAL
+    torch.cuda.synchronize()
+    assert torch.equal(buf, before)                                            # a failed call changes nothing
+
+
+def test_kv_append_tokens_equals_the_reference_scatter(oracle):
+    # tail step: new tokens' K/V go straight into the pool ("appending one new entry")
+    rng = np.random.default_rng(11)
+    NL, Hkv, d, Hq, nb = 2, 8, 128, 32, 80
+    q_lens = [1, 37, 0, 1, 16, 1]
+    kv_lens = [1, 100, 50, 160, 16, 33]
+    image = np.full(oracle.pool_elems(NL, nb, Hkv, d), GUARD, dtype=np.uint16)
+    order = synth.shuffled_free_order(rng, nb)
+    tables, pos = [], 0
+    for t in kv_lens:
+        n = synth.blocks_for(t)
+        tables.append(order[pos:pos + n])
+        pos += n
+    total_q = sum(q_lens)
+    Kn = synth.random_bits(rng, (NL, total_q, Hkv, d))
+    Vn = synth.random_bits(rng, (NL, total_q, Hkv, d))
+    expected, r = image.copy(), 0
+    for b, m in enumerate(q_lens):
+        if m:
+            expected = oracle.scatter(expected, NL, nb, Hkv, d, Kn[:, r:r + m], Vn[:, r:r + m], m, kv_lens[b] - m, tables[b])
+            r += m
+    d_image = u16_dev(image)
+    pool = B.KvPool(B.pool_desc(NL, nb, Hkv, d), d_image)
+    shape = B.attn_shape(Hq, Hkv, d)
+    ws = torch.empty(B.csv_plan_workspace_bytes(shape, q_lens, kv_lens), dtype=torch.uint8, device="cuda")
+    plan = B.Plan(shape, q_lens, kv_lens, 0, ws)
+    tabs, mb = synth.dense_tables(tables)
+    B.kv_append_tokens(pool, plan, u16_dev(Kn), u16_dev(Vn), dev(tabs), mb)
+    torch.cuda.synchronize()
+    assert np.array_equal(dev_to_u16(d_image), expected)
