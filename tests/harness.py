@@ -121,7 +121,11 @@ def assert_close(O, LSE, O_ref, LSE_ref, what="", norm=True):
     assert np.all(np.isfinite(O)), "%s: non-finite O" % what
     assert np.all(np.isfinite(LSE)), "%s: non-finite LSE" % what
     err = np.abs(O - O_ref)
-    assert err.max() <= O_TOL, "%s: max |O err| %.3e > %.0e" % (what, err.max(), O_TOL)
+    # north_star's absolute bound is stated for "outputs O(1)": a bf16 output near 3 already rounds by 2^-7 = 7.8e-3.
+    # Rows whose reference exceeds 1 in magnitude (a handful of visible keys) get the same bound relative to |O|_inf.
+    scale = np.maximum(1.0, np.abs(O_ref).max(axis=-1, keepdims=True))
+    worst = (err / scale).max()
+    assert worst <= O_TOL, "%s: max |O err| %.3e (scaled %.3e) > %.0e" % (what, err.max(), worst, O_TOL)
     lerr = np.abs(LSE - LSE_ref).max()
     assert lerr <= LSE_TOL, "%s: max |LSE err| %.3e > %.0e" % (what, lerr, LSE_TOL)
     if norm:

@@ -77,7 +77,7 @@ def test_decode_spike_sweep_sees_every_block(oracle):
     """one key carries ~all the weight and its V is a +-1 pattern; sweeping the
     spike over every block boundary makes a dropped / misplaced block an O(1) error."""
     rng = np.random.default_rng(37)
-    Hq, Hkv, d, L = 32, 8, 128, 6000
+    Hq, Hkv, d, L = 32, 8, 128, 6001
     positions = sorted(set([0, 1, 15, 16, 17, L - 1, L - 2, (L // 16) * 16, (L // 16) * 16 - 1] +
                            list(range(16 * 7, L, 16 * 29)) + list(range(16 * 11 - 1, L, 16 * 31)) +
                            list(rng.integers(0, L, size=16))))
