@@ -229,7 +229,7 @@ def tail_extra(k, iters=10):
 def run_ours(args):
     import torch
     from paper_2606_01839_b200 import binding as B
-    from paper_2606_01839_b200 import workloads
+    from paper_2606_01839_b200 import replicas, workloads
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -244,7 +244,7 @@ def run_ours(args):
     B.lib()   # fails loudly if libconserve_kv.so is missing: there is no fallback
 
     # replicas only: rank r serves its own conversations (same length recipe, different seed)
-    wl = workloads.config_tail_workload(2, seed=1 + 100 * rank)
+    wl = workloads.config_tail_workload(2, seed=replicas.rank_seed(1, rank))
     kv_bytes = wl.decode_kv_bytes()
     rows = len(wl.kv_lens)
     K, W = args.steps, max(3, args.warmup)
@@ -283,15 +283,10 @@ def run_ours(args):
         torch.cuda.synchronize()
         t1 = time.time()
     clocks = sampler.stop(t0, t1) if sampler else None
-    if dist:
-        t = torch.tensor([ms_total], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
-        t = torch.tensor([dec_ms], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dec_ms = float(t.item())
+    ms_total, _ = replicas.aggregate(dist, ms_total, kv_bytes, device="cuda")
+    dec_ms, total_kv_bytes = replicas.aggregate(dist, dec_ms, kv_bytes, device="cuda")
     ms_step = ms_total / K
-    value = world * kv_bytes / ms_step / 1e6            # GB/s, whole job
+    value = total_kv_bytes / ms_step / 1e6              # GB/s, whole job (sum of bytes / max time)
     info = wl.plan.info()
     launches_per_step = 1 + 1 + (1 if info["n_decode_items"] > rows * wl.Hkv else 0)   # append_tokens, decode, merge
 
@@ -315,10 +310,7 @@ def run_ours(args):
         e2e_call()          # synchronises its stream before returning (the result is on the host)
     torch.cuda.synchronize()
     e2e_ms = (time.perf_counter() - tw) * 1e3 / K
-    if dist:
-        t = torch.tensor([e2e_ms], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item())
+    e2e_ms, _ = replicas.aggregate(dist, e2e_ms, kv_bytes, device="cuda")
     h2d = h_q.numel() * 2 + h_k.numel() * 2 + h_v.numel() * 2 + h_t.numel() * 4
     d2h = h_out.numel() * 2 + h_lse.numel() * 4
 
@@ -343,7 +335,7 @@ def run_ours(args):
         "roofline": {"bound": "hbm", "kernel": "decode_kernel<128,3> (+ decode_merge_kernel), per paged_decode_attn call",
                      "achieved": achieved, "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": achieved / peak,
                      "frac_of_nominal_8000": achieved / NOMINAL_HBM_GBS, "avg_launch_ms": dec_ms, "traffic": None},
-        "e2e": {"value": world * kv_bytes / e2e_ms / 1e6, "unit": UNIT, "ms_per_step": e2e_ms, "h2d_bytes_per_step": h2d,
+        "e2e": {"value": total_kv_bytes / e2e_ms / 1e6, "unit": UNIT, "ms_per_step": e2e_ms, "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "timing": "wall clock around csv_tail_step_host (host plan + copies + kernels + sync)"},
         "gpu_launches": launches_per_step * K, "clocks": clocks,
         "context": "paper (4xA40, Qwen3-0.6B): p95 TTFET -51.08 %, +7.51 % tokens/J vs AMPD (PAPER.md:7) - scheduling figures, not this path",

@@ -1,0 +1,133 @@
+"""Parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times
+(device-generated pools, the library's allocator with a shuffled free list, default plans), on
+sampled outputs the oracle can compute one by one.  The oracle reads the sampled conversations
+back from the pool image through its own gather (O2): no expected value comes from the CUDA path.
+"""
+import numpy as np
+import pytest
+import torch
+
+from paper_2606_01839_b200 import binding as B
+from paper_2606_01839_b200 import synth, workloads
+from harness import assert_close, bf16_dev_to_f64, dev_to_u16
+
+pytestmark = pytest.mark.gpu
+
+
+def free_gb():
+    return torch.cuda.mem_get_info()[0] / 1e9
+
+
+def check_rows(oracle, wl, layer, samples, O, LSE, what):
+    """samples: list of (conversation b, row index i inside its q rows).  Oracle on the truncated cache."""
+    starts = np.concatenate([[0], np.cumsum(wl.q_lens)])
+    q_all = dev_to_u16(wl.d_q).reshape(-1, wl.Hq, wl.d)
+    cache = {}
+    for b, i in samples:
+        if b not in cache:
+            cache = {b: wl.logical_kv(oracle, b, layer)}     # keep one conversation at a time (131k tokens = 512 MiB)
+        K, V = cache[b]
+        m = wl.q_lens[b]
+        n = wl.kv_lens[b] - m + i + 1                        # keys visible to row i (decode: m = 1, i = 0, n = kv_len)
+        r = starts[b] + i
+        o_ref, l_ref = oracle.attention(q_all[r:r + 1], K[:n], V[:n])
+        assert_close(O[r:r + 1], LSE[r:r + 1], o_ref, l_ref, what="%s conv %d row %d (n=%d)" % (what, b, i, n))
+
+
+def test_config3_agentic_tail_mix_full_size(oracle):
+    # BASELINE.json config 3: 256 conversations, lognormal prefixes, 224 decode rows + 32 chunks of m ~ U[32,512]
+    wl = workloads.config_tail_workload(3)
+    info = wl.plan.info()
+    assert info["n_decode_rows"] == 224 and info["n_append_chunks"] == 32
+    wl.d_out.fill_(0x7FC0)
+    wl.d_lse.fill_(float("nan"))
+    wl.decode()
+    wl.append()
+    torch.cuda.synchronize()
+    O, LSE = bf16_dev_to_f64(wl.d_out), wl.d_lse.cpu().numpy().astype(np.float64)
+    assert np.all(np.isfinite(O)) and np.all(np.isfinite(LSE))          # every row of both calls was written
+    dec = [b for b in range(256) if wl.q_lens[b] == 1]
+    app = [b for b in range(256) if wl.q_lens[b] > 1]
+    by_len = sorted(dec, key=lambda b: wl.kv_lens[b])
+    samples = [(b, 0) for b in (by_len[0], by_len[1], by_len[len(by_len) // 2], by_len[-1], dec[0], dec[-1])]
+    a_small = sorted(app, key=lambda b: wl.kv_lens[b])[:3] + [max(app, key=lambda b: wl.q_lens[b])]
+    for b in a_small:
+        m = wl.q_lens[b]
+        samples += [(b, 0), (b, m // 2), (b, m - 1)]
+    check_rows(oracle, wl, 0, samples, O, LSE, "config 3")
+
+
+def test_config5_long_context_full_size_eight_layers(oracle):
+    # BASELINE.json config 5: Hq=64, Hkv=8, d=128, 8 layers, 16 x 131072 tokens (~69 GB of KV), >= 64 partitions per sequence
+    if free_gb() < 90:
+        pytest.skip("needs ~75 GB of free device memory")
+    wl = workloads.config_tail_workload(5, layers=8)
+    assert wl.pool_bytes >= 64 * 2 ** 30
+    items, _ = wl.plan.decode_items()
+    assert np.bincount(items[:, 0], minlength=16).min() >= 64 * 8
+    app = wl.with_q_lens(workloads.config5_append_q_lens())
+    for layer in (0, 7):                                     # layer 7 starts 56 GiB into the pool: 64-bit addressing
+        wl.d_out.fill_(0x7FC0)
+        wl.decode(layer=layer)
+        torch.cuda.synchronize()
+        O, LSE = bf16_dev_to_f64(wl.d_out), wl.d_lse.cpu().numpy().astype(np.float64)
+        assert np.all(np.isfinite(O))
+        check_rows(oracle, wl, layer, [(3 if layer == 0 else 15, 0)], O, LSE, "config 5 decode layer %d" % layer)
+    app.d_out.fill_(0x7FC0)
+    app.append(layer=7)
+    torch.cuda.synchronize()
+    O, LSE = bf16_dev_to_f64(app.d_out), app.d_lse.cpu().numpy().astype(np.float64)
+    assert np.all(np.isfinite(O))
+    check_rows(oracle, app, 7, [(2, 0), (2, 255)], O, LSE, "config 5 append layer 7")
+
+
+def test_config4_handoff_full_size(oracle):
+    # BASELINE.json config 4: 16 conversations x 32 layers of 8B-shape KV, random 16-bit patterns, batched pack -> unpack
+    if free_gb() < 75:
+        pytest.skip("needs ~65 GB of free device memory")
+    cfg = synth.CONFIGS[4]
+    toks = [int(t) for t in synth.config_lengths(4)["tokens"]]
+    NL, Hkv, d = cfg["NL"], cfg["Hkv"], cfg["d"]
+    rng = np.random.default_rng(cfg["seed"])
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(44)
+    nb = synth.pool_blocks_for(toks, slack=0.10)
+    desc = B.pool_desc(NL, nb, Hkv, d)
+    GUARD = -23101                                           # 0xA5C3 as int16
+    d_pool = torch.full((B.kv_pool_bytes(desc) // 2,), GUARD, dtype=torch.int16, device="cuda")
+    pool = B.KvPool(desc, d_pool)
+    pool.set_free_order(synth.shuffled_free_order(rng, nb))
+    ks, vs, sts, ids, h_ids = [], [], [], [], []
+    for t in toks:
+        n = NL * t * Hkv * d
+        ks.append(torch.randint(-32768, 32767, (n,), dtype=torch.int16, device="cuda", generator=gen).view(NL, t, Hkv, d))
+        vs.append(torch.randint(-32768, 32767, (n,), dtype=torch.int16, device="cuda", generator=gen).view(NL, t, Hkv, d))
+        sts.append(torch.full((B.kv_staging_bytes(desc, t) // 2,), 0x1111, dtype=torch.int16, device="cuda"))
+        h_ids.append(pool.alloc_blocks(synth.blocks_for(t)))
+        ids.append(torch.from_numpy(h_ids[-1]).cuda())
+    B.kv_pack_batch(desc, ks, vs, toks, [0] * 16, sts)
+    B.kv_unpack_batch(pool, sts, toks, [0] * 16, ids, [len(i) for i in h_ids])
+    torch.cuda.synchronize()
+    unit = 2 * Hkv * 16 * d                                   # int16 elements of one (layer, block)
+    pool_v = d_pool.view(NL, nb, unit)
+    srng = np.random.default_rng(5)
+    for c in [int(np.argmin(toks)), int(np.argmax(toks))] + list(srng.integers(0, 16, size=4)):
+        t = toks[c]
+        ntb = synth.blocks_for(t)
+        for layer, tb in [(0, 0), (NL - 1, ntb - 1)] + [(int(srng.integers(0, NL)), int(srng.integers(0, ntb))) for _ in range(6)]:
+            lo, hi = tb * 16, min(t, tb * 16 + 16)
+            K = dev_to_u16(ks[c][layer, lo:hi]).reshape(1, hi - lo, Hkv, d)
+            V = dev_to_u16(vs[c][layer, lo:hi]).reshape(1, hi - lo, Hkv, d)
+            msg = oracle.staging_message(1, Hkv, d, K, V, hi - lo, 0)            # the 64 KiB unit, unused slots zero
+            got_st = dev_to_u16(sts[c].view(NL, ntb, unit)[layer, tb])
+            assert np.array_equal(got_st, msg), "staging unit (conv %d, layer %d, block %d)" % (c, layer, tb)
+            expect_pool = oracle.scatter(np.full(unit, 0xA5C3, dtype=np.uint16), 1, 1, Hkv, d, K, V, hi - lo, 0,
+                                         np.zeros(1, dtype=np.int32))            # unused slots keep the guard
+            got_pool = dev_to_u16(pool_v[layer, int(h_ids[c][tb])])
+            assert np.array_equal(got_pool, expect_pool), "pool unit (conv %d, layer %d, block %d)" % (c, layer, tb)
+    # blocks never handed out are untouched, in every layer
+    used = np.zeros(nb, dtype=bool)
+    used[np.concatenate(h_ids)] = True
+    free_ids = torch.from_numpy(np.flatnonzero(~used)[:64].astype(np.int64)).cuda()
+    assert bool((pool_v[:, free_ids] == GUARD).all())
+    assert pool.used_blocks == sum(synth.blocks_for(t) for t in toks)
