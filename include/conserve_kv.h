@@ -215,9 +215,10 @@ int kv_append_tokens(kv_pool_t* dst, const csv_plan_t* plan, const void* d_k_new
  * decode row, q_len m > 1 = appended chunk with prefix P = kv_len - m.
  *
  * Split-K: the flattened (conversation, block) stream of the q_len = 1 rows is
- * cut into one contiguous share per CTA, and each share into partitions of at
- * most max_partition_tokens tokens (a multiple of 16; 0 = default 2048) that
- * never cross a conversation.  The schedule depends only on the lengths, so
+ * cut into one contiguous share per warp-worker (8 per CTA), and each share into
+ * partitions that never cross a (conversation, KV head) boundary and, if
+ * max_partition_tokens > 0 (a multiple of 16), hold at most that many tokens
+ * (0 = no extra cut).  The schedule depends only on the lengths, so
  * results are bit-identical under any block permutation and from run to run.
  * ---------------------------------------------------------------------- */
 

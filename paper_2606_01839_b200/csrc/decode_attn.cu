@@ -18,10 +18,12 @@
 //    512 B of KV, 68-99 % of the FP32 issue rate at G = 8; HMMA makes
 //    the arithmetic ~8 % of issue slots so the kernel stays on the HBM roofline.
 //  * Online softmax in fp32 in the log2 domain; P rounded to bf16 for the PV product; each
-//    partition leaves (o, m, l) fp32 partials, merged in a fixed order by merge_kernel
-//    (deterministic, no float atomics).  Single-partition (conversation, head) pairs write
-//    O / LSE directly.
+//    partition leaves (o, m, l) fp32 partials, merged in partial-index order (deterministic, no
+//    float atomics) by decode_merge_kernel.  (An in-kernel last-arriver merge was measured slower:
+//    the __threadfence + atomic per partition cost 12 us on config 2 against 6 us for the launch.)
+//    Single-partition (conversation, head) pairs write O / LSE directly.
 #include <math.h>
+#include <stdlib.h>
 
 #include "common.cuh"
 #include "internal.h"
@@ -41,6 +43,37 @@ struct DecodeParams {
     int32_t max_blocks, Hq, Hkv, G;
     float scale_log2;
 };
+
+// One warp per (merge group, query head of the group): log-sum-exp merge of the group's partials in
+// partial-index order (deterministic, no float atomics).
+template <int D>
+__global__ void __launch_bounds__(128) decode_merge_kernel(const MergeGroup* __restrict__ groups, int n_groups, int G,
+                                                           int Hq, const float* __restrict__ po,
+                                                           const float* __restrict__ pml, uint16_t* out, float* lse) {
+    constexpr int VEC = D / 32;
+    const int w = blockIdx.x * 4 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (w >= n_groups * G) return;
+    const MergeGroup g = groups[w / G];
+    const int hh = w % G;
+    float M = -INFINITY;
+    for (int k = 0; k < g.count; ++k) M = fmaxf(M, __ldg(pml + ((size_t)(g.first + k) * G + hh) * 2));
+    float L = 0.f, acc[VEC];
+#pragma unroll
+    for (int v = 0; v < VEC; ++v) acc[v] = 0.f;
+    for (int k = 0; k < g.count; ++k) {
+        const float2 ml = __ldg(reinterpret_cast<const float2*>(pml + ((size_t)(g.first + k) * G + hh) * 2));
+        const float wgt = fast_exp2(ml.x - M);
+        L += ml.y * wgt;
+        const float* src = po + ((size_t)(g.first + k) * G + hh) * D + lane * VEC;
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) acc[v] += __ldg(src + v) * wgt;
+    }
+    const float inv = 1.f / L;
+    uint16_t* orow = out + ((size_t)g.q_start * Hq + (size_t)g.head * G + hh) * D + lane * VEC;
+#pragma unroll
+    for (int v = 0; v < VEC; v += 2) *reinterpret_cast<uint32_t*>(orow + v) = pack_bf16(acc[v] * inv, acc[v + 1] * inv);
+    if (lane == 0) lse[(size_t)g.q_start * Hq + (size_t)g.head * G + hh] = (M + log2f(L)) * 0.6931471805599453f;
+}
 
 template <int D, int STAGES>
 __global__ void __launch_bounds__(kDecodeWarps * 32, 1) decode_kernel(const __grid_constant__ DecodeParams p) {
@@ -71,14 +104,28 @@ __global__ void __launch_bounds__(kDecodeWarps * 32, 1) decode_kernel(const __gr
 
     uint32_t cnt = 0;   // blocks consumed so far by this warp (ring position)
     const int item_begin = __ldg(p.worker_begin + worker), item_end = __ldg(p.worker_begin + worker + 1);
+    int4 c0 = make_int4(0, 0, 0, 0), c1 = c0, c2 = c0, n0 = c0, n1 = c0, n2 = c0;
+    if (item_begin < item_end) {
+        c0 = __ldg(reinterpret_cast<const int4*>(p.items + item_begin));
+        c1 = __ldg(reinterpret_cast<const int4*>(p.items + item_begin) + 1);
+        c2 = __ldg(reinterpret_cast<const int4*>(p.items + item_begin) + 2);
+    }
+    int ids_pref = 0;
+    bool have_pref = false;
     for (int ii = item_begin; ii < item_end; ++ii) {
-        const int4 i0 = __ldg(reinterpret_cast<const int4*>(p.items + ii));
-        const int4 i1 = __ldg(reinterpret_cast<const int4*>(p.items + ii) + 1);
-        const int conv = i0.x, head = i0.y, blk_begin = i0.z, blk_end = i0.w;
-        const int kv_len = i1.x, partial = i1.y, direct = i1.z, q_row = i1.w;
+        const int conv = c0.x, head = c0.y, blk_begin = c0.z, blk_end = c0.w;
+        const int kv_len = c1.x, partial = c1.y, direct = c1.z, q_row = c1.w;
         const int nblk = blk_end - blk_begin;
         const int32_t* tab = p.tables + (size_t)conv * p.max_blocks + blk_begin;
-        int ids_cur = lane < nblk ? __ldg(tab + lane) : 0;
+        int ids_cur = have_pref ? ids_pref : (lane < nblk ? __ldg(tab + lane) : 0);
+        have_pref = false;
+        const bool has_next = ii + 1 < item_end;
+        if (has_next) {   // next item's record: lands while this item streams
+            n0 = __ldg(reinterpret_cast<const int4*>(p.items + ii + 1));
+            n1 = __ldg(reinterpret_cast<const int4*>(p.items + ii + 1) + 1);
+            n2 = __ldg(reinterpret_cast<const int4*>(p.items + ii + 1) + 2);
+        }
+        const int pf_at = nblk > 3 ? nblk - 3 : 0;   // when to fetch the next item's first 32 block ids
         int ids_nxt = 32 + lane < nblk ? __ldg(tab + 32 + lane) : 0;
         int grp_cur = 0;
 
@@ -184,6 +231,11 @@ __global__ void __launch_bounds__(kDecodeWarps * 32, 1) decode_kernel(const __gr
                     bulk_g2s(dst + TB, src + kv_stride, TB, &bars[stage]);
                 }
             }
+            if (i == pf_at && has_next) {
+                const int nn = n0.w - n0.z;
+                ids_pref = lane < nn ? __ldg(p.tables + (size_t)n0.x * p.max_blocks + n0.z + lane) : 0;
+                have_pref = true;
+            }
             if (((i + 1) & 31) == 0) {
                 ids_cur = ids_nxt;
                 ++grp_cur;
@@ -195,52 +247,25 @@ __global__ void __launch_bounds__(kDecodeWarps * 32, 1) decode_kernel(const __gr
         // epilogue
         l_run += __shfl_xor_sync(0xffffffffu, l_run, 1);
         l_run += __shfl_xor_sync(0xffffffffu, l_run, 2);
-        if (row < G) {
-            if (direct) {
+        if (direct) {
+            if (row < G) {
                 const float inv = 1.f / l_run;
                 uint16_t* orow = p.out + ((size_t)q_row * p.Hq + (size_t)head * G + row) * D;
 #pragma unroll
                 for (int n = 0; n < NT; ++n)
                     *reinterpret_cast<uint32_t*>(orow + n * 8 + 2 * t4) = pack_bf16(o[n][0] * inv, o[n][1] * inv);
                 if (t4 == 0) p.lse[(size_t)q_row * p.Hq + (size_t)head * G + row] = (m_run + log2f(l_run)) * 0.6931471805599453f;
-            } else {
+            }
+        } else {
+            if (row < G) {
                 float* orow = p.po + ((size_t)partial * G + row) * D;
 #pragma unroll
                 for (int n = 0; n < NT; ++n) *reinterpret_cast<float2*>(orow + n * 8 + 2 * t4) = make_float2(o[n][0], o[n][1]);
                 if (t4 == 0) *reinterpret_cast<float2*>(p.pml + ((size_t)partial * G + row) * 2) = make_float2(m_run, l_run);
             }
         }
+        c0 = n0, c1 = n1, c2 = n2;
     }
-}
-
-// One warp per (merge group, query head of the group).  Fixed order => deterministic.
-template <int D>
-__global__ void __launch_bounds__(128) decode_merge_kernel(const MergeGroup* groups, int n_groups, int G, int Hq,
-                                                           const float* po, const float* pml, uint16_t* out,
-                                                           float* lse) {
-    constexpr int VEC = D / 32;
-    const int w = blockIdx.x * 4 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
-    if (w >= n_groups * G) return;
-    const MergeGroup g = groups[w / G];
-    const int hh = w % G;
-    float M = -INFINITY;
-    for (int k = 0; k < g.count; ++k) M = fmaxf(M, __ldg(pml + ((size_t)(g.first + k) * G + hh) * 2));
-    float L = 0.f, acc[VEC];
-#pragma unroll
-    for (int v = 0; v < VEC; ++v) acc[v] = 0.f;
-    for (int k = 0; k < g.count; ++k) {
-        const float2 ml = __ldg(reinterpret_cast<const float2*>(pml + ((size_t)(g.first + k) * G + hh) * 2));
-        const float wgt = fast_exp2(ml.x - M);
-        L += ml.y * wgt;
-        const float* src = po + ((size_t)(g.first + k) * G + hh) * D + lane * VEC;
-#pragma unroll
-        for (int v = 0; v < VEC; ++v) acc[v] += __ldg(src + v) * wgt;
-    }
-    const float inv = 1.f / L;
-    uint16_t* orow = out + ((size_t)g.q_start * Hq + (size_t)g.head * G + hh) * D + lane * VEC;
-#pragma unroll
-    for (int v = 0; v < VEC; v += 2) *reinterpret_cast<uint32_t*>(orow + v) = pack_bf16(acc[v] * inv, acc[v + 1] * inv);
-    if (lane == 0) lse[(size_t)g.q_start * Hq + (size_t)g.head * G + hh] = (M + log2f(L)) * 0.6931471805599453f;
 }
 
 template <int D, int STAGES>

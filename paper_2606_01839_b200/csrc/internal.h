@@ -22,7 +22,7 @@ struct kv_pool {
 
 static inline size_t csv_tile_bytes(int d) { return (size_t)CSV_BLOCK_SIZE * d * 2; }
 
-// ---- work lists (device-visible, 32-byte records) ---------------------------------------
+// ---- work lists (device-visible, 16-byte-aligned records) ---------------------------------------
 // One decode partition: blocks [blk_begin, blk_end) of conversation `conv`, KV head `head`.
 struct DecodeItem {
     int32_t conv;
@@ -33,6 +33,10 @@ struct DecodeItem {
     int32_t partial;   // index into the decode partial arrays
     int32_t direct;    // 1 = the only partition of its (conv, head): write O / LSE directly
     int32_t q_row;     // row of this conversation in d_q / d_out / d_lse (= sum of earlier q_lens)
+    int32_t group;        // index of the (conv, head) merge group, -1 if direct
+    int32_t group_first;  // first partial of the group
+    int32_t group_count;  // partials in the group
+    int32_t pad;
 };
 
 // One append work item: a tile of stacked rows (token-major: row r = i * G + hh) of one

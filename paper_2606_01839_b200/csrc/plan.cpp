@@ -6,8 +6,11 @@
 // the (conversation, KV head, block) stream of all q_len = 1 rows is flattened in that order
 // and cut into one contiguous share per WARP-worker (decode_grid CTAs x kDecodeWarps warps),
 // so every worker streams the same number of 8 KiB (K tile + V tile) units whatever the
-// length mix.  A share is cut further at (conversation, head) boundaries and every
-// max_partition_tokens tokens.  Each piece is one DecodeItem = one partial (o, m, l).
+// length mix.  A share is cut further at (conversation, head) boundaries and, if the caller asks for
+// it, every max_partition_tokens tokens (the default adds no cut: equal shares already balance the
+// load, and every extra partition is one more partial to merge).  Each piece is one DecodeItem = one
+// partial (o, m, l).  Config 5 (16 x 131072 tokens) still gets >= 64 partitions per sequence: each of
+// its 8 KV heads spans ~9.25 shares.
 // The schedule depends only on the lengths: results are bit-identical under any block
 // permutation and from run to run.
 #include <algorithm>
@@ -75,6 +78,7 @@ static void plan_decode(csv_plan* p) {
                 it.kv_len = p->kv_lens[b];
                 it.partial = -1;
                 it.direct = 0;
+                it.group = -1;
                 it.q_row = p->q_start[(size_t)b];
                 p->decode_items.push_back(it);
                 blk = end;
@@ -89,7 +93,13 @@ static void plan_decode(csv_plan* p) {
                 mg.conv = b;
                 mg.head = g;
                 mg.q_start = p->q_start[(size_t)b];
-                for (size_t i = 0; i < n; ++i) p->decode_items[first_item + i].partial = p->n_decode_partials++;
+                for (size_t i = 0; i < n; ++i) {
+                    DecodeItem& di = p->decode_items[first_item + i];
+                    di.partial = p->n_decode_partials++;
+                    di.group = (int32_t)p->decode_groups.size();
+                    di.group_first = mg.first;
+                    di.group_count = mg.count;
+                }
                 p->decode_groups.push_back(mg);
             }
             base += nblk;
@@ -237,7 +247,7 @@ csv_plan* csv_plan_build_host(const csv_attn_shape* shape, const int32_t* h_q_le
     p->shape = *shape;
     p->batch = batch;
     p->max_partition_tokens_user = max_partition_tokens;
-    p->max_partition_tokens = max_partition_tokens > 0 ? max_partition_tokens : 2048;
+    p->max_partition_tokens = max_partition_tokens > 0 ? max_partition_tokens : (1 << 30);   // 0: share cuts only
     p->num_sms = csv_query_num_sms();
     p->q_lens.assign(h_q_lens, h_q_lens + batch);
     p->kv_lens.assign(h_kv_lens, h_kv_lens + batch);
@@ -288,7 +298,7 @@ int32_t csv_plan_decode_items(const csv_plan_t* plan, int32_t* h_out, int32_t ma
     if (!plan) return -1;
     const int32_t n = (int32_t)plan->decode_items.size();
     if (h_out)
-        for (int32_t i = 0; i < n && i < max_items; ++i) memcpy(h_out + (size_t)i * 8, &plan->decode_items[(size_t)i], 32);
+        for (int32_t i = 0; i < n && i < max_items; ++i) memcpy(h_out + (size_t)i * 8, &plan->decode_items[(size_t)i], 32);   // first 8 fields
     if (h_worker_begin)
         for (int32_t i = 0; i < (int32_t)plan->worker_begin.size() && i < max_workers_plus_1; ++i)
             h_worker_begin[i] = plan->worker_begin[(size_t)i];

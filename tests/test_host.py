@@ -165,7 +165,7 @@ def check_decode_plan(q_lens, kv_lens, Hq, Hkv, d, mpt=0):
     items, wb = plan.decode_items()
     W = info["decode_grid"] * 8
     assert wb[0] == 0 and wb[W] == len(items) and np.all(np.diff(wb) >= 0)
-    cap = (mpt if mpt else 2048) // 16
+    cap = (mpt if mpt else 1 << 30) // 16
     # every (conv, head, block) of every q_len = 1 row is covered exactly once, in order
     cover = {}
     for conv, head, b0, b1, kv_len, partial, direct, _ in items:
@@ -207,7 +207,9 @@ def test_decode_plan_covers_config_shapes():
     plan, info = check_decode_plan([1] * 16, [131072] * 16, 64, 8, 128)
     items, _ = plan.decode_items()
     per_seq = np.bincount(items[:, 0], minlength=16)
-    assert per_seq.min() >= 64 * 8        # >= 64 partitions per (sequence, KV head)
+    assert per_seq.min() >= 64            # >= 64 partitions per sequence (8 KV heads x >= 9 shares each)
+    plan64, _ = check_decode_plan([1] * 16, [131072] * 16, 64, 8, 128, mpt=2048)
+    assert np.bincount(plan64.decode_items()[0][:, 0], minlength=16).min() >= 64 * 8   # forced: >= 64 per (sequence, head)
 
 
 def test_decode_plan_edge_lengths_and_partition_sizes():
