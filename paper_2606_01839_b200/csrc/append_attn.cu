@@ -267,27 +267,27 @@ __global__ void __launch_bounds__(kAppendWarps * 32, 2) append_kernel(const __gr
 
 // One warp per (merge group, tile row).
 template <int D>
-__global__ void __launch_bounds__(128) append_merge_kernel(const MergeGroup* groups, int n_groups, int G, int Hq,
+__global__ void __launch_bounds__(128) append_merge_kernel(const MergeGroup* groups, int n_groups, int TR, int G, int Hq,
                                                            const float* po, const float* pml, uint16_t* out,
                                                            float* lse) {
     constexpr int VEC = D / 32;
     const int w = blockIdx.x * 4 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
-    if (w >= n_groups * kAppendTileRows) return;
-    const MergeGroup g = groups[w / kAppendTileRows];
-    const int tr = w % kAppendTileRows;
+    if (w >= n_groups * TR) return;
+    const MergeGroup g = groups[w / TR];
+    const int tr = w % TR;
     const int r = g.row_begin + tr;
     if (r >= g.m * G) return;
     float M = -INFINITY;
-    for (int k = 0; k < g.count; ++k) M = fmaxf(M, __ldg(pml + ((size_t)(g.first + k) * kAppendTileRows + tr) * 2));
+    for (int k = 0; k < g.count; ++k) M = fmaxf(M, __ldg(pml + ((size_t)(g.first + k) * TR + tr) * 2));
     float L = 0.f, acc[VEC];
 #pragma unroll
     for (int v = 0; v < VEC; ++v) acc[v] = 0.f;
     for (int k = 0; k < g.count; ++k) {
-        const float2 ml = __ldg(reinterpret_cast<const float2*>(pml + ((size_t)(g.first + k) * kAppendTileRows + tr) * 2));
+        const float2 ml = __ldg(reinterpret_cast<const float2*>(pml + ((size_t)(g.first + k) * TR + tr) * 2));
         if (ml.x == -INFINITY) continue;   // this partition held no visible key for the row
         const float wgt = fast_exp2(ml.x - M);
         L += ml.y * wgt;
-        const float* src = po + ((size_t)(g.first + k) * kAppendTileRows + tr) * D + lane * VEC;
+        const float* src = po + ((size_t)(g.first + k) * TR + tr) * D + lane * VEC;
 #pragma unroll
         for (int v = 0; v < VEC; ++v) acc[v] += __ldg(src + v) * wgt;
     }
@@ -312,12 +312,17 @@ int launch_append_t(const csv_plan* plan, const AppendParams& p, cudaStream_t st
     const int grid = p.n_items < cap ? p.n_items : cap;
     append_kernel<D><<<grid, kAppendWarps * 32, smem, stream>>>(p);
     CSV_CUDA_TRY(cudaGetLastError());
+    return CSV_OK;
+}
+
+template <int D>
+int launch_append_merge(const csv_plan* plan, const AppendParams& p, cudaStream_t stream) {
     const int ng = (int)plan->append_groups.size();
     if (ng > 0) {
-        const int warps = ng * kAppendTileRows;
+        const int warps = ng * plan->append_tile_rows;
         append_merge_kernel<D><<<(warps + 3) / 4, 128, 0, stream>>>(
-            reinterpret_cast<const MergeGroup*>(plan->d_ws + plan->lay.append_groups), ng, p.G, p.Hq, p.po, p.pml, p.out,
-            p.lse);
+            reinterpret_cast<const MergeGroup*>(plan->d_ws + plan->lay.append_groups), ng, plan->append_tile_rows, p.G,
+            p.Hq, p.po, p.pml, p.out, p.lse);
         CSV_CUDA_TRY(cudaGetLastError());
     }
     return CSV_OK;
@@ -344,6 +349,13 @@ int launch_append_attn(const csv_plan* plan, const kv_pool* pool, int layer, con
     p.Hkv = plan->shape.num_kv_heads;
     p.G = p.Hq / p.Hkv;
     p.scale_log2 = (float)(1.4426950408889634 / sqrt((double)s.head_dim));
-    if (s.head_dim == 128) return launch_append_t<128>(plan, p, (cudaStream_t)stream);
-    return launch_append_t<64>(plan, p, (cudaStream_t)stream);
+    if (s.head_dim == 128) {
+        // d = 128: tcgen05 / TMEM kernel (append_attn_tc.cu), 128-row tiles
+        const int rc = launch_append_attn_tc(plan, pool, layer, q, tables, max_blocks, out, lse, stream);
+        if (rc != CSV_OK) return rc;
+        return launch_append_merge<128>(plan, p, (cudaStream_t)stream);
+    }
+    const int rc = launch_append_t<64>(plan, p, (cudaStream_t)stream);
+    if (rc != CSV_OK) return rc;
+    return launch_append_merge<64>(plan, p, (cudaStream_t)stream);
 }

@@ -111,6 +111,7 @@ static void plan_decode(csv_plan* p) {
 static void plan_append(csv_plan* p) {
     const int Hkv = p->shape.num_kv_heads;
     const int G = p->shape.num_q_heads / Hkv;
+    const int TR = p->append_tile_rows = p->shape.head_dim == 128 ? kAppendTileRowsTc : kAppendTileRows;
     p->n_append_chunks = 0;
     p->n_append_rows = 0;
     p->append_items.clear();
@@ -130,8 +131,8 @@ static void plan_append(csv_plan* p) {
             if (m <= 1) continue;
             const int P = p->kv_lens[b] - m;
             const int rows = m * G;
-            for (int r0 = 0; r0 < rows; r0 += kAppendTileRows) {
-                const int i_max = std::min(m - 1, (std::min(rows, r0 + kAppendTileRows) - 1) / G);
+            for (int r0 = 0; r0 < rows; r0 += TR) {
+                const int i_max = std::min(m - 1, (std::min(rows, r0 + TR) - 1) / G);
                 const int nblk = (P + i_max + 1 + CSV_BLOCK_SIZE - 1) / CSV_BLOCK_SIZE;
                 n += (int64_t)Hkv * ((nblk + split_blocks - 1) / split_blocks);
             }
@@ -154,8 +155,8 @@ static void plan_append(csv_plan* p) {
         const int P = p->kv_lens[b] - m;
         const int rows = m * G;
         for (int g = 0; g < Hkv; ++g)
-            for (int r0 = 0; r0 < rows; r0 += kAppendTileRows) {
-                const int i_max = std::min(m - 1, (std::min(rows, r0 + kAppendTileRows) - 1) / G);
+            for (int r0 = 0; r0 < rows; r0 += TR) {
+                const int i_max = std::min(m - 1, (std::min(rows, r0 + TR) - 1) / G);
                 const int nblk = (P + i_max + 1 + CSV_BLOCK_SIZE - 1) / CSV_BLOCK_SIZE;
                 const int nparts = (nblk + split_blocks - 1) / split_blocks;
                 MergeGroup mg{};
@@ -212,8 +213,8 @@ static void plan_layout(csv_plan* p) {
     const size_t list_bytes = off;
     L.decode_po = take((size_t)p->n_decode_partials * G * d * sizeof(float));
     L.decode_pml = take((size_t)p->n_decode_partials * G * 2 * sizeof(float));
-    L.append_po = take((size_t)p->n_append_partials * kAppendTileRows * d * sizeof(float));
-    L.append_pml = take((size_t)p->n_append_partials * kAppendTileRows * 2 * sizeof(float));
+    L.append_po = take((size_t)p->n_append_partials * p->append_tile_rows * d * sizeof(float));
+    L.append_pml = take((size_t)p->n_append_partials * p->append_tile_rows * 2 * sizeof(float));
     L.total = std::max<size_t>(off, 128);
     p->h_image.assign(list_bytes, 0);
     auto put = [&](size_t at, const void* src, size_t bytes) {
