@@ -82,6 +82,20 @@ int kv_unpack(kv_pool_t* dst, const void* d_staging, int32_t tokens, int32_t tok
     return kv_unpack_batch(dst, 1, &d_staging, &tokens, &token_offset, &d_block_ids, &n_ids, stream);
 }
 
+// Points a host-built plan at its device workspace and enqueues the upload of its work lists.
+static int plan_attach(csv_plan* p, void* d_workspace, size_t ws_bytes, void* stream) {
+    if (!aligned(d_workspace, 128)) return CSV_E_INVAL;
+    if (ws_bytes < p->lay.total) return CSV_E_NOMEM;
+    p->d_ws = (uint8_t*)d_workspace;
+    if (!p->h_image.empty()) {
+        // pageable source: the runtime stages it before returning, so h_image may be reused freely
+        cudaError_t e = cudaMemcpyAsync(d_workspace, p->h_image.data(), p->h_image.size(), cudaMemcpyHostToDevice,
+                                        (cudaStream_t)stream);
+        if (e != cudaSuccess) return csv_set_cuda_error((int)e);
+    }
+    return CSV_OK;
+}
+
 int csv_plan_create(const csv_attn_shape* shape, const int32_t* h_q_lens, const int32_t* h_kv_lens, int32_t batch,
                     int32_t max_partition_tokens, void* d_workspace, size_t ws_bytes, void* stream, csv_plan_t** out) {
     if (!out) return CSV_E_INVAL;
@@ -89,23 +103,10 @@ int csv_plan_create(const csv_attn_shape* shape, const int32_t* h_q_lens, const 
     csv_plan* p = csv_plan_build_host(shape, h_q_lens, h_kv_lens, batch, max_partition_tokens, &err);
     if (!p) return err;
     if (d_workspace) {
-        if (!aligned(d_workspace, 128)) {
+        const int rc = plan_attach(p, d_workspace, ws_bytes, stream);
+        if (rc != CSV_OK) {
             delete p;
-            return CSV_E_INVAL;
-        }
-        if (ws_bytes < p->lay.total) {
-            delete p;
-            return CSV_E_NOMEM;
-        }
-        p->d_ws = (uint8_t*)d_workspace;
-        if (!p->h_image.empty()) {
-            // pageable source: the runtime stages it before returning, so h_image may be reused freely
-            cudaError_t e = cudaMemcpyAsync(d_workspace, p->h_image.data(), p->h_image.size(), cudaMemcpyHostToDevice,
-                                            (cudaStream_t)stream);
-            if (e != cudaSuccess) {
-                delete p;
-                return csv_set_cuda_error((int)e);
-            }
+            return rc;
         }
     }
     *out = p;
@@ -192,15 +193,22 @@ int csv_tail_step_host(kv_pool_t* pool, int32_t layer, const csv_attn_shape* sha
         !h_lse || !d_workspace || !aligned(d_workspace, 128) || max_blocks <= 0)
         return CSV_E_INVAL;
     std::vector<int32_t> ones((size_t)batch, 1);
-    const size_t pb = csv_plan_workspace_bytes(shape, ones.data(), h_kv_lens, batch, max_partition_tokens);
-    if (pb == 0) return CSV_E_INVAL;
+    int err;
+    csv_plan_t* plan = csv_plan_build_host(shape, ones.data(), h_kv_lens, batch, max_partition_tokens, &err);   // planned once
+    if (!plan) return err;
+    const size_t pb = plan->lay.total;
     const TailLayout L = tail_layout(shape, batch, max_blocks, pb);
-    if (ws_bytes < L.total) return CSV_E_NOMEM;
+    if (ws_bytes < L.total) {
+        csv_plan_destroy(plan);
+        return CSV_E_NOMEM;
+    }
     uint8_t* ws = (uint8_t*)d_workspace;
     cudaStream_t st = (cudaStream_t)stream;
-    csv_plan_t* plan = nullptr;
-    int rc = csv_plan_create(shape, ones.data(), h_kv_lens, batch, max_partition_tokens, ws + L.plan, pb, stream, &plan);
-    if (rc != CSV_OK) return rc;
+    int rc = plan_attach(plan, ws + L.plan, pb, stream);
+    if (rc != CSV_OK) {
+        csv_plan_destroy(plan);
+        return rc;
+    }
     const size_t qb = (size_t)batch * shape->num_q_heads * shape->head_dim * 2;
     const size_t kb = (size_t)batch * shape->num_kv_heads * shape->head_dim * 2;
     cudaError_t e;

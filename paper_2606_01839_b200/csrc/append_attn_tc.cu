@@ -218,20 +218,24 @@ __global__ void __launch_bounds__(kTcThreads, 2) append_tc_kernel(const __grid_c
                 // visible columns of this chunk for this row (<= 0: none).  Columns past the blocks actually loaded
                 // hold stale shared memory and are masked too (a KV partition may end before the row's limit).
                 const int nvis = min(lim - tok0 + 1, nb * 16);
+                // raw scores stay unscaled: max on the raw values (scale > 0), and the scale folds into the
+                // exponent's FFMA below: p = exp2(s * scale - ref)
                 float x[64];
 #pragma unroll
                 for (int k = 0; k < 32; ++k) {
-                    x[k] = __uint_as_float(s0[k]) * p.scale_log2;
-                    x[32 + k] = __uint_as_float(s1[k]) * p.scale_log2;
+                    x[k] = __uint_as_float(s0[k]);
+                    x[32 + k] = __uint_as_float(s1[k]);
                 }
                 if (nvis < kChunk) {
 #pragma unroll
                     for (int k = 0; k < 64; ++k)
                         if (k >= nvis) x[k] = -INFINITY;
                 }
-                float mx = x[0];
+                float mraw = x[0];
 #pragma unroll
-                for (int k = 1; k < 64; ++k) mx = fmaxf(mx, x[k]);
+                for (int k = 1; k < 63; k += 2) mraw = fmax3(mraw, x[k], x[k + 1]);
+                mraw = fmaxf(mraw, x[63]);
+                const float mx = mraw * p.scale_log2;   // -inf stays -inf
                 if (j == 0) {
                     m_used = mx;   // PV_0 overwrites O (accumulate = 0): nothing to rescale yet
                 } else {
@@ -256,13 +260,16 @@ __global__ void __launch_bounds__(kTcThreads, 2) append_tc_kernel(const __grid_c
                 }
                 const float ref = m_used == -INFINITY ? 0.f : m_used;
                 uint32_t pk[32];
-                float lsum = 0.f;
+                const float2 sc2 = make_float2(p.scale_log2, p.scale_log2), nref2 = make_float2(-ref, -ref);
+                float2 acc2 = make_float2(0.f, 0.f);
 #pragma unroll
                 for (int k = 0; k < 32; ++k) {
-                    const float p0 = fast_exp2(x[2 * k] - ref), p1 = fast_exp2(x[2 * k + 1] - ref);
-                    lsum += p0 + p1;
+                    const float2 t = ffma2(make_float2(x[2 * k], x[2 * k + 1]), sc2, nref2);
+                    const float p0 = fast_exp2(t.x), p1 = fast_exp2(t.y);
+                    acc2 = fadd2(acc2, make_float2(p0, p1));
                     pk[k] = pack_bf16(p0, p1);
                 }
+                const float lsum = acc2.x + acc2.y;
                 l_run += lsum;
                 tmem_st32(lane_base + b * 64, pk);   // P_j over the first 32 columns of S_j (this lane's row only)
                 tmem_wait_st();
