@@ -250,8 +250,11 @@ def run_ours(args):
     K, W = args.steps, max(3, args.warmup)
 
     def step():
-        wl.kv_append_tokens()
-        wl.decode()
+        if args.unfused:
+            wl.kv_append_tokens()
+            wl.decode()
+        else:
+            wl.decode_step()   # paged_decode_step: the new token's K/V write fused into the decode launch
 
     for _ in range(W):
         step()
@@ -312,7 +315,7 @@ def run_ours(args):
     ms_step = ms_total / K
     value = total_kv_bytes / ms_step / 1e6              # GB/s, whole job (sum of bytes / max time)
     info = wl.plan.info()
-    launches_per_step = 3   # append_tokens_kernel + decode_kernel + decode_merge_kernel
+    launches_per_step = 3 if args.unfused else 2   # [append_tokens_kernel +] decode_kernel + decode_merge_kernel
 
     # end to end through the C-ABI call with HOST buffers (plan + H2D + kernels + D2H inside the timed region)
     pin = lambda t: t.cpu().pin_memory()
@@ -349,7 +352,7 @@ def run_ours(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms_step,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
         "config": {"workload": "configs[1] c2_llama8b_decode64: Hq=32 Hkv=8 d=128 bs=16, 64 conversations, context U[1024,8192], "
-                               "shuffled paged pool; step = kv_append_tokens + paged_decode_attn",
+                               "shuffled paged pool; step = " + ("kv_append_tokens + paged_decode_attn" if args.unfused else "paged_decode_step (new-token KV write fused into the decode launch)"),
                    "kv_bytes_per_step_per_gpu": kv_bytes, "kv_tokens": int(sum(wl.kv_lens)), "decode_rows": rows,
                    "l2": "inputs larger than L2 (%.2f GB of KV per step vs 126 MB)" % (kv_bytes / 1e9),
                    "parallelism": "replicas x%d, no collective" % world, "decode_grid": info["decode_grid"],
@@ -399,6 +402,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-extras", action="store_true")
     ap.add_argument("--no-graph", action="store_true")
+    ap.add_argument("--unfused", action="store_true", help="kv_append_tokens + paged_decode_attn as two calls")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

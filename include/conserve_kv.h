@@ -277,6 +277,17 @@ int paged_decode_attn(const csv_plan_t* plan, const kv_pool_t* pool, int32_t lay
                       const int32_t* d_block_tables, int32_t max_blocks, void* d_out, float* d_lse,
                       void* stream);
 
+/* Fused decode tail step (§2.1: decode "generates each subsequent token by reading the
+ * full KV cache and appending one new entry"): kv_append_tokens for the q_len = 1 rows of ONE layer
+ * and paged_decode_attn in a single launch.  d_k_new, d_v_new: this layer's new-token K / V,
+ * [total_q][Hkv][d] bf16 (rows of conversations with q_len != 1 are ignored: use kv_append_tokens
+ * for appended chunks).  The warp that streams a conversation's last block patches the new token's
+ * rows into the landed tiles and writes them to the pool at position kv_len - 1; results and all
+ * other arguments are exactly those of kv_append_tokens followed by paged_decode_attn. */
+int paged_decode_step(const csv_plan_t* plan, kv_pool_t* pool, int32_t layer, const void* d_q,
+                      const void* d_k_new, const void* d_v_new, const int32_t* d_block_tables,
+                      int32_t max_blocks, void* d_out, float* d_lse, void* stream);
+
 /* ------------------------------------------------------------------------
  * a5. append_prefill_attn.  PAPER.md:94 §3.1: "relatively small prompts are
  * appended to the whole history context ... only calculating new KV cache
@@ -298,7 +309,7 @@ int append_prefill_attn(const csv_plan_t* plan, const kv_pool_t* pool, int32_t l
  * decode tail step of one layer.  Plans from the host lengths, copies
  * h_q, h_k_new, h_v_new ([batch][Hq|Hkv][d] bf16, one new token per
  * conversation, already counted in h_kv_lens) and h_block_tables to the
- * device workspace, runs kv_append_tokens + paged_decode_attn, copies O and
+ * device workspace, runs paged_decode_step (= kv_append_tokens + paged_decode_attn), copies O and
  * LSE back to h_out / h_lse and synchronises `stream`.
  * d_workspace: >= csv_tail_step_host_workspace_bytes(...), 128-byte aligned.
  * ---------------------------------------------------------------------- */

@@ -21,7 +21,8 @@ int csv_query_num_sms() {
         return n;
     }
     (void)cudaGetLastError();
-    return 148;   // B200; lets the planner run on a box without a GPU (host tests)
+    cached = 148;   // B200; lets the planner run on a box without a GPU (host tests)
+    return cached;
 }
 
 static bool aligned(const void* p, size_t a) { return ((uintptr_t)p & (a - 1)) == 0; }
@@ -134,6 +135,15 @@ int paged_decode_attn(const csv_plan_t* plan, const kv_pool_t* pool, int32_t lay
     return launch_decode(plan, pool, layer, d_q, d_block_tables, max_blocks, d_out, d_lse, stream);
 }
 
+int paged_decode_step(const csv_plan_t* plan, kv_pool_t* pool, int32_t layer, const void* d_q, const void* d_k_new,
+                      const void* d_v_new, const int32_t* d_block_tables, int32_t max_blocks, void* d_out, float* d_lse,
+                      void* stream) {
+    const int rc = check_attn_args(plan, pool, layer, d_q, d_block_tables, max_blocks, d_out, d_lse);
+    if (rc != CSV_OK) return rc;
+    if (!d_k_new || !d_v_new || !aligned(d_k_new, 16) || !aligned(d_v_new, 16)) return CSV_E_INVAL;
+    return launch_decode(plan, pool, layer, d_q, d_block_tables, max_blocks, d_out, d_lse, stream, d_k_new, d_v_new);
+}
+
 int append_prefill_attn(const csv_plan_t* plan, const kv_pool_t* pool, int32_t layer, const void* d_q,
                         const int32_t* d_block_tables, int32_t max_blocks, void* d_out, float* d_lse, void* stream) {
     const int rc = check_attn_args(plan, pool, layer, d_q, d_block_tables, max_blocks, d_out, d_lse);
@@ -226,11 +236,9 @@ int csv_tail_step_host(kv_pool_t* pool, int32_t layer, const csv_attn_shape* sha
     layer_view.d_base = pool->d_base + (size_t)layer * pool->desc.num_blocks * 2 * pool->desc.num_kv_heads *
                                            csv_tile_bytes(pool->desc.head_dim);
     if (layer < 0 || layer >= pool->desc.num_layers) rc = CSV_E_INVAL;
-    if (rc == CSV_OK)
-        rc = kv_append_tokens(&layer_view, plan, ws + L.k, ws + L.v, (const int32_t*)(ws + L.tables), max_blocks, stream);
-    if (rc == CSV_OK)
-        rc = paged_decode_attn(plan, &layer_view, 0, ws + L.q, (const int32_t*)(ws + L.tables), max_blocks, ws + L.out,
-                               (float*)(ws + L.lse), stream);
+    if (rc == CSV_OK)   // new-token KV write fused into the decode launch
+        rc = paged_decode_step(plan, &layer_view, 0, ws + L.q, ws + L.k, ws + L.v, (const int32_t*)(ws + L.tables), max_blocks,
+                               ws + L.out, (float*)(ws + L.lse), stream);
     if (rc == CSV_OK) {
         if ((e = cudaMemcpyAsync(h_out, ws + L.out, qb, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
             (e = cudaMemcpyAsync(h_lse, ws + L.lse, (size_t)batch * shape->num_q_heads * 4, cudaMemcpyDeviceToHost, st)) !=

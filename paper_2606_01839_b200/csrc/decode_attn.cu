@@ -40,6 +40,9 @@ struct DecodeParams {
     float* lse;
     float* po;
     float* pml;
+    const uint8_t* k_new;   // fused step only: this layer's new-token K / V, [total_q][Hkv][d] bf16, else NULL
+    const uint8_t* v_new;
+    uint8_t* pool_layer_w;  // same address as pool_layer, writable (fused step)
     int32_t max_blocks, Hq, Hkv, G;
     float scale_log2;
 };
@@ -52,8 +55,10 @@ __global__ void __launch_bounds__(128) decode_merge_kernel(const MergeGroup* __r
                                                            const float* __restrict__ pml, uint16_t* out, float* lse) {
     constexpr int VEC = D / 32;
     const int w = blockIdx.x * 4 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    MergeGroup g = {};
+    if (w < n_groups * G) g = groups[w / G];   // plan data, not decode_kernel output
+    pdl_wait();                                // partials are complete and visible
     if (w >= n_groups * G) return;
-    const MergeGroup g = groups[w / G];
     const int hh = w % G;
     float M = -INFINITY;
     for (int k = 0; k < g.count; ++k) M = fmaxf(M, __ldg(pml + ((size_t)(g.first + k) * G + hh) * 2));
@@ -112,6 +117,9 @@ __global__ void __launch_bounds__(kDecodeWarps * 32, 1) decode_kernel(const __gr
     }
     int ids_pref = 0;
     bool have_pref = false;
+    // Plan data (work lists) was read above; tables, Q and the pool may come from the previous kernel.
+    pdl_wait();
+    pdl_trigger();   // decode_merge_kernel may be scheduled now; it waits for this grid to finish
     for (int ii = item_begin; ii < item_end; ++ii) {
         const int conv = c0.x, head = c0.y, blk_begin = c0.z, blk_end = c0.w;
         const int kv_len = c1.x, partial = c1.y, direct = c1.z, q_row = c1.w;
@@ -165,6 +173,24 @@ __global__ void __launch_bounds__(kDecodeWarps * 32, 1) decode_kernel(const __gr
             mbar_wait(&bars[stage], parity);
             const uint32_t kt = ring_u32 + stage * 2 * TB, vt = kt + TB;
             const int nvalid = kv_len - (blk_begin + i) * 16;   // >= 1; < 16 only in the conversation's last block
+            if (p.k_new != nullptr && nvalid <= 16) {
+                // Fused tail step ("reading the full KV cache and appending one new entry"): this warp owns
+                // the conversation's last block for this head.  The new token's K / V rows go into the landed tiles
+                // (so this step attends to them) and into the pool (so the cache has grown).  Nobody else reads this
+                // (block, head) in this launch, and the bulk copy that read the old bytes has completed.
+                const int slot = nvalid - 1;
+                const int c = lane & 15, kv = lane >> 4;   // lanes 0-15: K row chunks, 16-31: V row chunks
+                const int id = __shfl_sync(0xffffffffu, ids_cur, i & 31);   // block i is in the current id group
+                if (c < D / 8) {
+                    const uint4 val = *reinterpret_cast<const uint4*>((kv ? p.v_new : p.k_new) +
+                                                                      ((size_t)q_row * p.Hkv + head) * (D * 2) + c * 16);
+                    const uint32_t off = (uint32_t)((c >> 3) * 2048 + slot * 128 + (((c & 7) ^ (slot & 7)) << 4));
+                    *reinterpret_cast<uint4*>(ring + (size_t)stage * 2 * TB + kv * TB + off) = val;
+                    *reinterpret_cast<uint4*>(p.pool_layer_w + (size_t)head * TB + (size_t)id * blk_stride + kv * kv_stride + off) = val;
+                }
+                fence_proxy_async();
+                __syncwarp();
+            }
             if (nvalid < 16) {
                 // slots past kv_len may hold anything (NaN patterns): 0 * NaN must not reach the PV accumulators
                 uint8_t* vtile = ring + (size_t)stage * 2 * TB + TB;
@@ -277,15 +303,13 @@ int launch_decode_t(const csv_plan* plan, const DecodeParams& p, cudaStream_t st
         CSV_CUDA_TRY(cudaFuncSetAttribute(decode_kernel<D, STAGES>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_set = true;
     }
-    decode_kernel<D, STAGES><<<plan->decode_grid, kDecodeWarps * 32, smem, stream>>>(p);
-    CSV_CUDA_TRY(cudaGetLastError());
+    CSV_CUDA_TRY(launch_pdl(decode_kernel<D, STAGES>, dim3(plan->decode_grid), dim3(kDecodeWarps * 32), smem, stream, p));
     const int ng = (int)plan->decode_groups.size();
     if (ng > 0) {
         const int warps = ng * p.G;
-        decode_merge_kernel<D><<<(warps + 3) / 4, 128, 0, stream>>>(
-            reinterpret_cast<const MergeGroup*>(plan->d_ws + plan->lay.decode_groups), ng, p.G, p.Hq, p.po, p.pml, p.out,
-            p.lse);
-        CSV_CUDA_TRY(cudaGetLastError());
+        CSV_CUDA_TRY(launch_pdl(decode_merge_kernel<D>, dim3((warps + 3) / 4), dim3(128), 0, stream,
+                                reinterpret_cast<const MergeGroup*>(plan->d_ws + plan->lay.decode_groups), ng, p.G, p.Hq,
+                                (const float*)p.po, (const float*)p.pml, p.out, p.lse));
     }
     return CSV_OK;
 }
@@ -293,7 +317,7 @@ int launch_decode_t(const csv_plan* plan, const DecodeParams& p, cudaStream_t st
 }   // namespace
 
 int launch_decode(const csv_plan* plan, const kv_pool* pool, int layer, const void* q, const int32_t* tables,
-                  int max_blocks, void* out, float* lse, void* stream) {
+                  int max_blocks, void* out, float* lse, void* stream, const void* k_new, const void* v_new) {
     if (plan->decode_items.empty()) return CSV_OK;
     const kv_pool_desc& s = pool->desc;
     DecodeParams p;
@@ -306,6 +330,9 @@ int launch_decode(const csv_plan* plan, const kv_pool* pool, int layer, const vo
     p.lse = lse;
     p.po = reinterpret_cast<float*>(plan->d_ws + plan->lay.decode_po);
     p.pml = reinterpret_cast<float*>(plan->d_ws + plan->lay.decode_pml);
+    p.k_new = (const uint8_t*)k_new;
+    p.v_new = (const uint8_t*)v_new;
+    p.pool_layer_w = const_cast<uint8_t*>(p.pool_layer);
     p.max_blocks = max_blocks;
     p.Hq = plan->shape.num_q_heads;
     p.Hkv = plan->shape.num_kv_heads;

@@ -147,6 +147,7 @@ __global__ void __launch_bounds__(kThreads) append_tokens_kernel(uint8_t* pool, 
                                                                  const int32_t* tables, int max_blocks) {
     constexpr int CPR = D / 8;
     constexpr int TB = 16 * D * 2;
+    pdl_trigger();   // a PDL-launched paged_decode_attn may start its prologue; it waits for this grid
     const int32_t* q_start = meta;
     const int32_t* kv_len = meta + batch + 1;
     const int32_t* q_len = kv_len + batch;

@@ -115,7 +115,8 @@ int launch_unpack(kv_pool* dst, int n, const void* const* staging, const int32_t
 int launch_append_tokens(kv_pool* dst, const csv_plan* plan, const void* k_new, const void* v_new,
                          const int32_t* tables, int max_blocks, void* stream);
 int launch_decode(const csv_plan* plan, const kv_pool* pool, int layer, const void* q, const int32_t* tables,
-                  int max_blocks, void* out, float* lse, void* stream);
+                  int max_blocks, void* out, float* lse, void* stream, const void* k_new = nullptr,
+                  const void* v_new = nullptr);
 int launch_append_attn(const csv_plan* plan, const kv_pool* pool, int layer, const void* q, const int32_t* tables,
                        int max_blocks, void* out, float* lse, void* stream);
 int launch_append_attn_tc(const csv_plan* plan, const kv_pool* pool, int layer, const void* q, const int32_t* tables,

@@ -48,6 +48,7 @@ static void plan_decode(csv_plan* p) {
     const int64_t W = (int64_t)p->decode_grid * kDecodeWarps;
     p->worker_begin.assign((size_t)W + 1, 0);
     p->decode_items.clear();
+    p->decode_items.reserve((size_t)W + (size_t)p->n_decode_rows * Hkv + 16);
     p->decode_groups.clear();
     p->n_decode_partials = 0;
     if (units == 0) return;

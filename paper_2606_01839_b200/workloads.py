@@ -88,6 +88,12 @@ class TailWorkload:
         B.paged_decode_attn(self.plan, self.pool, layer, self.d_q, self.d_tables, self.max_blocks, self.d_out, self.d_lse,
                             stream)
 
+    def decode_step(self, layer=0, stream=None):
+        """Fused tail step: new-token K/V write + decode attention in one launch (decode rows only)."""
+        per_layer = self.total_q * self.Hkv * self.d
+        B.paged_decode_step(self.plan, self.pool, layer, self.d_q, self.d_k_new[layer * per_layer:],
+                            self.d_v_new[layer * per_layer:], self.d_tables, self.max_blocks, self.d_out, self.d_lse, stream)
+
     def append(self, layer=0, stream=None):
         B.append_prefill_attn(self.plan, self.pool, layer, self.d_q, self.d_tables, self.max_blocks, self.d_out,
                               self.d_lse, stream)

@@ -98,3 +98,35 @@ def test_tail_step_host_buffers(oracle):
     O = synth.bf16_bits_to_f32(h_out.numpy().view(np.uint16)).astype(np.float64)
     O_ref, LSE_ref = oracle_attention(sc, [1] * 5, q)
     assert_close(O, h_lse.numpy().astype(np.float64), O_ref, LSE_ref, what="tail step")
+
+
+@pytest.mark.parametrize("Hq,Hkv,d", [(32, 8, 128), (64, 8, 128), (4, 1, 64)])
+def test_fused_decode_step_writes_the_token_and_attends_to_it(oracle, Hq, Hkv, d):
+    """paged_decode_step = kv_append_tokens + paged_decode_attn in one launch: the pool must end up bit-identical to
+    the oracle's scatter of the full conversations, and O / LSE must match the oracle on the full cache."""
+    rng = np.random.default_rng(70 + d + Hq)
+    kv_lens = [1, 16, 17, 33, 2049, 640, 100, 4097]
+    n = len(kv_lens)
+    sc = Scenario(oracle, rng, Hq, Hkv, d, kv_lens, poison=True)
+    full = sc.image.copy()
+    for b, t in enumerate(kv_lens):
+        full = oracle.scatter(full, 1, sc.num_blocks, Hkv, d, sc.K[b], sc.V[b], t, 0, sc.tables[b])
+        if t > 1:   # the cache before the step: everything but the newest token
+            sc.image = oracle.scatter(sc.image, 1, sc.num_blocks, Hkv, d, sc.K[b][:, :t - 1], sc.V[b][:, :t - 1], t - 1, 0,
+                                      sc.tables[b])
+    sc.upload()
+    k_new = np.stack([sc.K[b][0, kv_lens[b] - 1] for b in range(n)])
+    v_new = np.stack([sc.V[b][0, kv_lens[b] - 1] for b in range(n)])
+    q = synth.normal_bf16(rng, (n, Hq, d))
+    shape = B.attn_shape(Hq, Hkv, d)
+    ws = torch.empty(B.csv_plan_workspace_bytes(shape, [1] * n, kv_lens), dtype=torch.uint8, device="cuda")
+    plan = B.Plan(shape, [1] * n, kv_lens, 0, ws)
+    d_out = torch.full((n, Hq, d), 0x7FC0, dtype=torch.int16, device="cuda")
+    d_lse = torch.full((n, Hq), float("nan"), dtype=torch.float32, device="cuda")
+    B.paged_decode_step(plan, sc.pool, 0, u16_dev(q), u16_dev(k_new), u16_dev(v_new), sc.d_tables, sc.max_blocks, d_out,
+                        d_lse)
+    torch.cuda.synchronize()
+    from harness import dev_to_u16
+    assert np.array_equal(dev_to_u16(sc.d_image), full), "pool after the fused step differs from the oracle's scatter"
+    O_ref, LSE_ref = oracle_attention(sc, [1] * n, q)
+    assert_close(bf16_dev_to_f64(d_out), d_lse.cpu().numpy().astype(np.float64), O_ref, LSE_ref, what="fused step")
