@@ -41,6 +41,23 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def ncu_traffic_bytes():
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of decode_kernel on this workload, from the committed
+    `ncu --set full` capture (profiles/r1_decode_ncu_full.csv); None if the file is not there."""
+    p = os.path.join(ROOT, "profiles", "r1_decode_ncu_full.csv")
+    unit = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+    try:
+        tot = 0.0
+        for line in open(p):
+            f = line.strip().split(",")
+            if f[0] in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+                vals = [float(x.strip('"')) for x in f[2:] if x]
+                tot += unit[f[1]] * sum(vals) / len(vals)
+        return tot or None
+    except Exception:
+        return None
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled DURING the timed region (profiling recipe)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -361,7 +378,9 @@ def run_ours(args):
         "pct_of_nominal_8000": 100.0 * value / world / NOMINAL_HBM_GBS,
         "roofline": {"bound": "hbm", "kernel": "decode_kernel<128,3> (+ decode_merge_kernel), per paged_decode_attn call; timed over K back-to-back calls",
                      "achieved": achieved, "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": achieved / peak,
-                     "frac_of_nominal_8000": achieved / NOMINAL_HBM_GBS, "avg_launch_ms": dec_ms, "traffic": None},
+                     "frac_of_nominal_8000": achieved / NOMINAL_HBM_GBS, "avg_launch_ms": dec_ms, "traffic": ncu_traffic_bytes(),
+                     "traffic_source": "profiles/r1_decode_ncu_full.csv (dram read + write bytes per decode_kernel launch)",
+                     "algorithmic_bytes": kv_bytes},
         "e2e": {"value": total_kv_bytes / e2e_ms / 1e6, "unit": UNIT, "ms_per_step": e2e_ms, "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "timing": "wall clock around csv_tail_step_host (host plan + copies + kernels + sync)"},
         "gpu_launches": launches_per_step * K, "clocks": clocks,
