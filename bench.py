@@ -3,10 +3,13 @@
 
 Default workload = BASELINE.json configs[1] (Llama-3-8B-shaped layer, 64 conversations,
 context U[1024,8192], block size 16, shuffled paged pool).  One STEP = one pass of the tail
-path over that batch: kv_append_tokens (the new token's K/V into the pool) + paged_decode_attn
-(split-K partitions + merge).  metric = KV bytes read / step time, in GB/s, whole job.
+path over that batch: paged_decode_step = the new token's K/V written into the pool + split-K paged
+decode attention + merge (--unfused: kv_append_tokens and paged_decode_attn as two calls), replayed
+from a CUDA graph (--no-graph: plain launches).  metric = KV bytes read / step time, in GB/s, whole job.
+The other configs (handoff, agentic tail mix, long context) are timed after the headline line's
+measurements and reported under "other_workloads" (--no-extras skips them).
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--no-extras]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--no-extras] [--no-graph] [--unfused]
 
 N > 1 (torchrun): replicas only — every rank serves its own pool of conversations,
 no data-path collective; barrier + max-over-ranks timing; value = total bytes / that time.

@@ -175,13 +175,13 @@ static TailLayout tail_layout(const csv_attn_shape* s, int batch, int max_blocks
         off = (off + b + 127) / 128 * 128;
         return at;
     };
-    L.plan = take(plan_bytes);
     L.q = take((size_t)batch * s->num_q_heads * s->head_dim * 2);
     L.k = take((size_t)batch * s->num_kv_heads * s->head_dim * 2);
     L.v = take((size_t)batch * s->num_kv_heads * s->head_dim * 2);
     L.tables = take((size_t)batch * max_blocks * 4);
     L.out = take((size_t)batch * s->num_q_heads * s->head_dim * 2);
     L.lse = take((size_t)batch * s->num_q_heads * 4);
+    L.plan = take(plan_bytes);   // last: its size is only known once the plan is built
     L.total = off;
     return L;
 }
@@ -202,40 +202,36 @@ int csv_tail_step_host(kv_pool_t* pool, int32_t layer, const csv_attn_shape* sha
     if (!pool || !shape || batch <= 0 || !h_kv_lens || !h_q || !h_k_new || !h_v_new || !h_block_tables || !h_out ||
         !h_lse || !d_workspace || !aligned(d_workspace, 128) || max_blocks <= 0)
         return CSV_E_INVAL;
-    std::vector<int32_t> ones((size_t)batch, 1);
-    int err;
-    csv_plan_t* plan = csv_plan_build_host(shape, ones.data(), h_kv_lens, batch, max_partition_tokens, &err);   // planned once
-    if (!plan) return err;
-    const size_t pb = plan->lay.total;
-    const TailLayout L = tail_layout(shape, batch, max_blocks, pb);
-    if (ws_bytes < L.total) {
-        csv_plan_destroy(plan);
-        return CSV_E_NOMEM;
-    }
-    uint8_t* ws = (uint8_t*)d_workspace;
-    cudaStream_t st = (cudaStream_t)stream;
-    int rc = plan_attach(plan, ws + L.plan, pb, stream);
-    if (rc != CSV_OK) {
-        csv_plan_destroy(plan);
-        return rc;
-    }
+    if (layer < 0 || layer >= pool->desc.num_layers) return CSV_E_INVAL;
+    // The plan's size is not known before it is built, so the fixed-size buffers sit in front of it: their copies
+    // are enqueued first and fly while the host plans.
     const size_t qb = (size_t)batch * shape->num_q_heads * shape->head_dim * 2;
     const size_t kb = (size_t)batch * shape->num_kv_heads * shape->head_dim * 2;
+    const TailLayout L = tail_layout(shape, batch, max_blocks, 0);   // L.plan is the END region here (see tail_layout)
+    if (ws_bytes < L.total) return CSV_E_NOMEM;
+    uint8_t* ws = (uint8_t*)d_workspace;
+    cudaStream_t st = (cudaStream_t)stream;
     cudaError_t e;
     if ((e = cudaMemcpyAsync(ws + L.q, h_q, qb, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
         (e = cudaMemcpyAsync(ws + L.k, h_k_new, kb, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
         (e = cudaMemcpyAsync(ws + L.v, h_v_new, kb, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
         (e = cudaMemcpyAsync(ws + L.tables, h_block_tables, (size_t)batch * max_blocks * 4, cudaMemcpyHostToDevice, st)) !=
-            cudaSuccess) {
-        csv_plan_destroy(plan);
+            cudaSuccess)
         return csv_set_cuda_error((int)e);
+    std::vector<int32_t> ones((size_t)batch, 1);
+    int err;
+    csv_plan_t* plan = csv_plan_build_host(shape, ones.data(), h_kv_lens, batch, max_partition_tokens, &err);   // planned once
+    if (!plan) return err;
+    int rc = ws_bytes - L.plan < plan->lay.total ? CSV_E_NOMEM : plan_attach(plan, ws + L.plan, ws_bytes - L.plan, stream);
+    if (rc != CSV_OK) {
+        csv_plan_destroy(plan);
+        return rc;
     }
     // the new token's K/V go to `layer` of the pool: view that layer as a 1-layer pool
     kv_pool layer_view = *pool;
     layer_view.desc.num_layers = 1;
     layer_view.d_base = pool->d_base + (size_t)layer * pool->desc.num_blocks * 2 * pool->desc.num_kv_heads *
                                            csv_tile_bytes(pool->desc.head_dim);
-    if (layer < 0 || layer >= pool->desc.num_layers) rc = CSV_E_INVAL;
     if (rc == CSV_OK)   // new-token KV write fused into the decode launch
         rc = paged_decode_step(plan, &layer_view, 0, ws + L.q, ws + L.k, ws + L.v, (const int32_t*)(ws + L.tables), max_blocks,
                                ws + L.out, (float*)(ws + L.lse), stream);

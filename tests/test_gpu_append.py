@@ -25,7 +25,8 @@ def step_case(oracle, seed, Hq, Hkv, d, convs, mpt=0, poison=False, v_mean=0.0, 
     return assert_close(O, LSE, O_ref, LSE_ref, what or "step"), info
 
 
-@pytest.mark.parametrize("Hq,Hkv,d", [(32, 8, 128), (64, 8, 128), (4, 1, 64), (8, 8, 64), (16, 2, 128)])
+@pytest.mark.parametrize("Hq,Hkv,d", [(32, 8, 128), (64, 8, 128), (4, 1, 64), (8, 8, 64), (16, 2, 128), (8, 8, 128), (8, 4, 128),
+                                      (2, 1, 64)])
 def test_append_chunk_length_edge_cases(oracle, Hq, Hkv, d):
     # m in {2, 31, 32, 33, 512}, P = 0, prefixes not multiples of 16
     convs = [(0, 2), (0, 33), (100, 31), (1000, 32), (17, 33), (777, 2), (15, 16), (3, 100)]
