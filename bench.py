@@ -209,6 +209,25 @@ def handoff_extra(iters=5):
     return out
 
 
+def prefill_extra(iters=5):
+    """turn-1 prefill attention of a 32768-token prompt in 8192-token chunks through
+    append_prefill_attn (m = 8192, P = earlier chunks), 8B shape, one layer."""
+    import torch
+    from paper_2606_01839_b200 import workloads
+
+    wl = workloads.TailWorkload(32, 8, 128, [1], [32768], seed=22)
+    total_ms, flops = 0.0, 0.0
+    for P in (0, 8192, 16384, 24576):
+        app = wl.with_q_lens([8192], [P + 8192])
+        ms, _ = time_calls(app.append, iters)
+        total_ms += ms
+        flops += app.append_flops()
+    del wl, app
+    torch.cuda.empty_cache()
+    return {"workload": "turn-1 prefill attention, 32768 tokens in 4 chunks of 8192 (Hq=32 Hkv=8 d=128, one layer)",
+            "ms": total_ms, "tflops": flops / total_ms / 1e9}
+
+
 def tail_extra(k, iters=10):
     """configs[2] (agentic tail mix) and configs[4] (70B-shaped long context, ONE of its 8 layers): per-call times."""
     import torch
@@ -403,7 +422,8 @@ def run_ours(args):
         if not args.no_extras:
             extras = {}
             for name, fn in (("handoff", handoff_extra), ("agentic_tail_mix", lambda: tail_extra(3)),
-                             ("long_context_70b", lambda: tail_extra(5))):
+                             ("long_context_70b", lambda: tail_extra(5)),
+                             ("turn1_prefill_chunked", prefill_extra)):
                 try:
                     extras[name] = fn()
                 except Exception as e:   # an extra must never cost the headline line

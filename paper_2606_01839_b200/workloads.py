@@ -58,11 +58,15 @@ class TailWorkload:
         self.plan = B.Plan(self.shape, self.q_lens, self.kv_lens, self.mpt, self.ws)
         torch.cuda.synchronize()
 
-    def with_q_lens(self, q_lens):
-        """Another step over the SAME pool and tables (e.g. config 5's append call next to its decode call)."""
+    def with_q_lens(self, q_lens, kv_lens=None):
+        """Another step over the SAME pool and tables (e.g. config 5's append call next to its decode call).
+        kv_lens (optional) may shorten the conversations: the pool simply holds more than the step looks at."""
         import copy
 
         other = copy.copy(self)
+        if kv_lens is not None:
+            assert all(int(a) <= int(b) for a, b in zip(kv_lens, self.kv_lens))
+            other.kv_lens = [int(x) for x in kv_lens]
         other._setup_queries(q_lens)
         return other
 

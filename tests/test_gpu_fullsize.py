@@ -131,3 +131,17 @@ def test_config4_handoff_full_size(oracle):
     free_ids = torch.from_numpy(np.flatnonzero(~used)[:64].astype(np.int64)).cuda()
     assert bool((pool_v[:, free_ids] == GUARD).all())
     assert pool.used_blocks == sum(synth.blocks_for(t) for t in toks)
+
+
+def test_turn1_prefill_chunk_8192_through_append_prefill_attn(oracle):
+    """turn-1 prefill attention, chunked 8192 tokens per batch as the paper configures the prefiller
+    (PAPER.md:213), is append_prefill_attn with m = 8192 and P = the tokens of the earlier chunks."""
+    wl = workloads.TailWorkload(32, 8, 128, [1], [16384], seed=21)
+    for P in (0, 8192):
+        app = wl.with_q_lens([8192], [P + 8192])
+        app.d_out.fill_(0x7FC0)
+        app.append()
+        torch.cuda.synchronize()
+        O, LSE = bf16_dev_to_f64(app.d_out), app.d_lse.cpu().numpy().astype(np.float64)
+        assert np.all(np.isfinite(O)) and np.all(np.isfinite(LSE))
+        check_rows(oracle, app, 0, [(0, 0), (0, 1), (0, 127), (0, 4096), (0, 8191)], O, LSE, "prefill chunk P=%d" % P)
