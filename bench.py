@@ -273,13 +273,22 @@ def run_ours(args):
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    local = local % max(1, torch.cuda.device_count())
     torch.cuda.set_device(local)
-    dist = None
+    dist, agg_dev = None, "cuda"
     if world > 1:
         import torch.distributed as dist_mod
 
         dist = dist_mod
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        try:   # the only cross-rank traffic is a barrier and scalar reductions (replicas, no data-path collective)
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+            dist.barrier()
+        except Exception as e:
+            sys.stderr.write("nccl unavailable (%r): using gloo for the barrier / scalar reductions\n" % (e,))
+            if dist.is_initialized():
+                dist.destroy_process_group()
+            dist.init_process_group("gloo")
+            agg_dev = "cpu"
     B.lib()   # fails loudly if libconserve_kv.so is missing: there is no fallback
 
     # replicas only: rank r serves its own conversations (same length recipe, different seed)
@@ -349,8 +358,8 @@ def run_ours(args):
         torch.cuda.synchronize()
         t1 = time.time()
     clocks = sampler.stop(t0, t1) if sampler else None
-    ms_total, _ = replicas.aggregate(dist, ms_total, kv_bytes, device="cuda")
-    dec_ms, total_kv_bytes = replicas.aggregate(dist, dec_ms, kv_bytes, device="cuda")
+    ms_total, _ = replicas.aggregate(dist, ms_total, kv_bytes, device=agg_dev)
+    dec_ms, total_kv_bytes = replicas.aggregate(dist, dec_ms, kv_bytes, device=agg_dev)
     ms_step = ms_total / K
     value = total_kv_bytes / ms_step / 1e6              # GB/s, whole job (sum of bytes / max time)
     info = wl.plan.info()
@@ -376,7 +385,7 @@ def run_ours(args):
         e2e_call()          # synchronises its stream before returning (the result is on the host)
     torch.cuda.synchronize()
     e2e_ms = (time.perf_counter() - tw) * 1e3 / K
-    e2e_ms, _ = replicas.aggregate(dist, e2e_ms, kv_bytes, device="cuda")
+    e2e_ms, _ = replicas.aggregate(dist, e2e_ms, kv_bytes, device=agg_dev)
     h2d = h_q.numel() * 2 + h_k.numel() * 2 + h_v.numel() * 2 + h_t.numel() * 4
     d2h = h_out.numel() * 2 + h_lse.numel() * 4
 
