@@ -251,7 +251,7 @@ int32_t csv_plan_decode_items(const csv_plan_t* plan, int32_t* h_out, int32_t ma
 /* Same for the append work list: item i is 12 int32 {conv, kv_head, row_begin,
  * q_start, m, kv_len, blk_begin, blk_end, partial, direct, 0, 0}; rows are the
  * m * G query rows of a chunk stacked token-major (row = token * G + head_in_group),
- * in tiles of 128 rows
+ * in tiles of 256 rows
  * (head_dim 128) or 64 rows (head_dim 64).  Returns the item count. */
 int32_t csv_plan_append_items(const csv_plan_t* plan, int32_t* h_out, int32_t max_items);
 

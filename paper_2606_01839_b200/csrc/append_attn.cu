@@ -350,8 +350,8 @@ int launch_append_attn(const csv_plan* plan, const kv_pool* pool, int layer, con
     p.G = p.Hq / p.Hkv;
     p.scale_log2 = (float)(1.4426950408889634 / sqrt((double)s.head_dim));
     if (s.head_dim == 128) {
-        // d = 128: tcgen05 / TMEM kernel (append_attn_tc.cu), 128-row tiles
-        const int rc = launch_append_attn_tc(plan, pool, layer, q, tables, max_blocks, out, lse, stream);
+        // d = 128: tcgen05 / TMEM kernel (append_attn_tc2.cu), two 128-row tiles per CTA
+        const int rc = launch_append_attn_tc2(plan, pool, layer, q, tables, max_blocks, out, lse, stream);
         if (rc != CSV_OK) return rc;
         return launch_append_merge<128>(plan, p, (cudaStream_t)stream);
     }

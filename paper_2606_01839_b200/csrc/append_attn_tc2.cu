@@ -1,0 +1,374 @@
+// append_attn_tc2.cu — append_prefill_attn for head_dim 128 on tcgen05 / TMEM, two row tiles per CTA.
+// PAPER.md:94 §3.1 / PAPER.md:60 §2.2 (see append_attn.cu).  Roofline: tensor (bf16, fp32 accumulate).
+//
+// One CTA per SM works on 256 stacked rows (token-major: row = token*G + head) of one KV head: two
+// 128-row tiles A and B that SHARE every K/V chunk.  Measured on the one-tile-per-CTA predecessor
+// (DESIGN.md §5): with two independent CTAs per SM the 2-stage K/V rings gave a stage one softmax
+// period of lead (< loaded L2/HBM latency) and every CTA re-read its own K/V.  Here the rings are 4
+// deep (two to three periods of lead), K/V traffic per row is halved, and the tensor pipe alternates
+// between the two tiles while the other tile's softmax runs.
+//   warps 0-3  softmax of tile A, warps 4-7 softmax of tile B (thread r owns row r = TMEM lane r % 128)
+//   warp 8     producer: 1-D bulk copies of K half-tiles / V tiles into the rings
+//   warps 9,10 MMA issuers, one per tile (a single issuing thread needs ~90 cycles per tcgen05.mma, measured: it was
+//              the bottleneck with 24 MMAs per chunk): S_t = Q_t K^T (SS, M=128, N=64), O_t += P_t V (A = P from TMEM)
+// TMEM (all 512 columns): tile t at t*256: S/P buffer 0 [0,64), buffer 1 [64,128), O [128,256).
+#include <math.h>
+
+#include "common.cuh"
+#include "internal.h"
+#include "tc5.cuh"
+
+namespace {
+
+constexpr int kT2Threads = 352;
+constexpr int kChunk = 64;                 // KV tokens per pipeline step
+constexpr int kChunkBlocks = kChunk / 16;
+constexpr int kKSt = 4, kVSt = 4;          // ring depths (16 KiB stages)
+constexpr uint32_t kTmemCols2 = 512;
+
+struct AppendTc2Params {
+    const AppendItem* items;
+    int32_t n_items;
+    const uint8_t* pool_layer;
+    const uint16_t* q;
+    const int32_t* tables;
+    uint16_t* out;
+    float* lse;
+    float* po;
+    float* pml;
+    int32_t max_blocks, Hq, Hkv, G;
+    float scale_log2;
+};
+
+constexpr uint32_t kOffQ2 = 0;                           // 2 tiles x [2 halves][128 rows][128 B]
+constexpr uint32_t kOffK2 = 65536;                       // kKSt x [2 halves][4 blocks][2048 B]
+constexpr uint32_t kOffV2 = kOffK2 + kKSt * 16384;       // kVSt x [4 blocks][4096 B]
+constexpr uint32_t kOffBar2 = kOffV2 + kVSt * 16384;     // mbarriers + TMEM slot
+constexpr uint32_t kSmemBytes2 = kOffBar2 + 256;
+
+__global__ void __launch_bounds__(kT2Threads, 1) append_tc2_kernel(const __grid_constant__ AppendTc2Params p) {
+    constexpr int D = 128;
+    constexpr int TB = 4096;
+    extern __shared__ __align__(1024) uint8_t smem[];
+    const uint32_t sbase = smem_u32(smem);
+    if (sbase & 1023u) __trap();   // SWIZZLE_128B operand tiles must be 1024-byte aligned
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + kOffBar2);
+    uint64_t *k_full = bars, *k_empty = bars + 4, *v_full = bars + 8, *v_empty = bars + 12;
+    uint64_t *s_full = bars + 16 /* [tile][buf] */, *p_full = bars + 20 /* [tile][buf] */, *o_done = bars + 24 /* [tile] */;
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 26);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < 4; ++i) {
+            mbar_init(&k_full[i], 1);
+            mbar_init(&k_empty[i], 2);   // both MMA warps release a stage
+            mbar_init(&v_full[i], 1);
+            mbar_init(&v_empty[i], 2);
+            mbar_init(&s_full[i], 1);
+            mbar_init(&p_full[i], 128);
+        }
+        mbar_init(&o_done[0], 1);
+        mbar_init(&o_done[1], 1);
+        fence_mbar_init();
+    }
+    if (warp == 9) tmem_alloc(tmem_slot, kTmemCols2);   // warp 9 also frees it
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = *tmem_slot;
+
+    const int G = p.G;
+    const size_t kv_stride = (size_t)p.Hkv * TB;
+    const size_t blk_stride = 2 * kv_stride;
+    uint32_t kc = 0;             // K/V chunks pushed through the rings so far (all roles agree)
+    uint32_t tcnA = 0, tcnB = 0;   // chunks each tile has processed so far (tile B skips items without rows for it)
+
+    for (int it = blockIdx.x; it < p.n_items; it += gridDim.x) {
+        const int4 i0 = __ldg(reinterpret_cast<const int4*>(p.items + it));
+        const int4 i1 = __ldg(reinterpret_cast<const int4*>(p.items + it) + 1);
+        const int4 i2 = __ldg(reinterpret_cast<const int4*>(p.items + it) + 2);
+        const int conv = i0.x, head = i0.y, row_begin = i0.z, q_start = i0.w;
+        const int m = i1.x, kv_len = i1.y, blk_begin = i1.z, blk_end = i1.w;
+        const int partial = i2.x, direct = i2.y;
+        const int P = kv_len - m;
+        const int rows_total = m * G;
+        const int nblk = blk_end - blk_begin;
+        const int nch = (nblk + kChunkBlocks - 1) / kChunkBlocks;
+        const bool hasB = row_begin + 128 < rows_total;
+
+        // ---- stage the Q rows of both tiles in the K-major SWIZZLE_128B image ------------------------
+        if (warp < 8) {
+            const int t = warp >> 2, r = threadIdx.x & 127, sr = row_begin + t * 128 + r;
+            if (t == 0 || hasB) {
+                const bool ok = sr < rows_total;
+                const uint4* src = reinterpret_cast<const uint4*>(
+                    p.q + ((size_t)(q_start + (ok ? sr / G : 0)) * p.Hq + (size_t)head * G + (ok ? sr % G : 0)) * D);
+                uint4 v[16];
+#pragma unroll
+                for (int c = 0; c < 16; ++c) v[c] = ok ? __ldg(src + c) : make_uint4(0, 0, 0, 0);
+#pragma unroll
+                for (int c = 0; c < 16; ++c)
+                    *reinterpret_cast<uint4*>(smem + kOffQ2 + t * 32768 + (c >> 3) * 16384 + r * 128 +
+                                              (((c & 7) ^ (r & 7)) << 4)) = v[c];
+                fence_proxy_async();
+            }
+        }
+        tc_fence_before();
+        __syncthreads();   // Q staged; the previous item's epilogues have finished reading O
+        tc_fence_after();
+
+        if (warp == 8) {
+            // ================= producer =================
+            if (lane == 0) {
+                const int32_t* tab = p.tables + (size_t)conv * p.max_blocks + blk_begin;
+                const uint8_t* head_base = p.pool_layer + (size_t)head * TB;
+                int ids[kChunkBlocks], nids[kChunkBlocks];
+#pragma unroll
+                for (int jb = 0; jb < kChunkBlocks; ++jb) nids[jb] = jb < nblk ? __ldg(tab + jb) : 0;
+                for (int j = 0; j < nch; ++j) {
+                    const uint32_t c = kc + j, ks = c % kKSt, kph = (c / kKSt) & 1, vs = c % kVSt, vph = (c / kVSt) & 1;
+                    const int nb = min(kChunkBlocks, nblk - j * kChunkBlocks);
+#pragma unroll
+                    for (int jb = 0; jb < kChunkBlocks; ++jb) {
+                        ids[jb] = nids[jb];
+                        const int nx = (j + 1) * kChunkBlocks + jb;
+                        nids[jb] = nx < nblk ? __ldg(tab + nx) : 0;
+                    }
+                    uint8_t* kb = smem + kOffK2 + ks * 16384;
+                    uint8_t* vb = smem + kOffV2 + vs * 16384;
+                    mbar_wait(&k_empty[ks], kph ^ 1);
+                    mbar_expect_tx(&k_full[ks], (uint32_t)nb * TB);
+#pragma unroll
+                    for (int jb = 0; jb < kChunkBlocks; ++jb)
+                        if (jb < nb) {
+                            const uint8_t* src = head_base + (size_t)ids[jb] * blk_stride;
+                            bulk_g2s(kb + jb * 2048, src, 2048, &k_full[ks]);
+                            bulk_g2s(kb + 8192 + jb * 2048, src + 2048, 2048, &k_full[ks]);
+                        }
+                    mbar_wait(&v_empty[vs], vph ^ 1);
+                    mbar_expect_tx(&v_full[vs], (uint32_t)nb * TB);
+#pragma unroll
+                    for (int jb = 0; jb < kChunkBlocks; ++jb)
+                        if (jb < nb)
+                            bulk_g2s(vb + jb * TB, head_base + (size_t)ids[jb] * blk_stride + kv_stride, TB, &v_full[vs]);
+                }
+            }
+        } else if (warp >= 9) {
+            // ================= MMA issuers: warp 9 -> tile A, warp 10 -> tile B =================
+            constexpr uint32_t idS = idesc_bf16(128, kChunk, 0, 0);
+            constexpr uint32_t idO = idesc_bf16(128, D, 0, 1);
+            const int t = warp - 9;
+            const bool active = t == 0 || hasB;      // an idle issuer still releases the K/V stages
+            const uint32_t tc0 = t ? tcnB : tcnA;
+            auto issue_S = [&](int j) {
+                const uint32_t c = kc + j, ks = c % kKSt, kph = (c / kKSt) & 1;
+                mbar_wait(&k_full[ks], kph);
+                tc_fence_after();
+                {
+                    if (active) {
+                        const uint32_t bt = (tc0 + j) & 1;
+#pragma unroll
+                        for (int hk = 0; hk < 8; ++hk) {   // hk = half * 4 + k-step inside the 64-element half
+                            const uint32_t off = (hk >> 2) * 16384 + (hk & 3) * 32;
+                            const uint32_t offk = (hk >> 2) * 8192 + (hk & 3) * 32;
+                            mma_ss_elect(tmem + t * 256 + bt * 64, smem_desc_sw128(sbase + kOffQ2 + t * 32768 + off, 16, 1024),
+                                   smem_desc_sw128(sbase + kOffK2 + ks * 16384 + offk, 16, 1024), idS, hk != 0);
+                        }
+                        tc_commit_elect(&s_full[t * 2 + bt]);
+                    }
+                    tc_commit_elect(&k_empty[ks]);
+                }
+                __syncwarp();
+            };
+            issue_S(0);
+            for (int j = 0; j < nch; ++j) {
+                if (j + 1 < nch) issue_S(j + 1);
+                const uint32_t c = kc + j, vs = c % kVSt, vph = (c / kVSt) & 1;
+                const int nb = min(kChunkBlocks, nblk - j * kChunkBlocks);
+                const uint32_t tcv = tc0 + j, bt = tcv & 1, pht = (tcv >> 1) & 1;
+                if (active) mbar_wait(&p_full[t * 2 + bt], pht);
+                mbar_wait(&v_full[vs], vph);
+                const int tok0 = (blk_begin + j * kChunkBlocks) * 16;
+                if (active && tok0 + nb * 16 > kv_len) {   // slots past kv_len may hold NaN patterns: 0 * NaN must not reach O
+                    // (both issuers write the same zeros; each fences its own writes before its own MMAs)
+                    const int nvalid = kv_len - (tok0 + (nb - 1) * 16);
+                    uint8_t* vt = smem + kOffV2 + vs * 16384 + (nb - 1) * TB;
+                    for (int cidx = lane; cidx < TB / 16; cidx += 32)
+                        if (((cidx & 127) >> 3) >= nvalid) *reinterpret_cast<uint4*>(vt + cidx * 16) = make_uint4(0, 0, 0, 0);
+                    fence_proxy_async();
+                    __syncwarp();
+                }
+                tc_fence_after();
+                {
+                    if (active) {
+                        for (int kk = 0; kk < nb; ++kk)
+                            mma_ts_elect(tmem + t * 256 + 128, tmem + t * 256 + bt * 64 + kk * 8,
+                                   smem_desc_sw128(sbase + kOffV2 + vs * 16384 + kk * TB, 2048, 1024), idO, (j | kk) != 0);
+                        tc_commit_elect(&o_done[t]);
+                    }
+                    tc_commit_elect(&v_empty[vs]);
+                }
+                __syncwarp();
+            }
+        } else {
+            // ================= softmax: warps 0-3 tile A, warps 4-7 tile B =================
+            const int t = warp >> 2;
+            if (t == 0 || hasB) {
+                const int r = threadIdx.x & 127, sr = row_begin + t * 128 + r;
+                const bool ok = sr < rows_total;
+                const int lim = ok ? P + sr / G : kv_len - 1;   // last visible key; rows past the chunk see all (Q = 0)
+                const uint32_t lane_base = tmem + t * 256 + ((uint32_t)((warp & 3) * 32) << 16);
+                const uint32_t tc0 = t ? tcnB : tcnA;
+                float m_used = -INFINITY, l_run = 0.f;
+                for (int j = 0; j < nch; ++j) {
+                    const uint32_t c = tc0 + j, b = c & 1, ph = (c >> 1) & 1;
+                    mbar_wait(&s_full[t * 2 + b], ph);
+                    tc_fence_after();
+                    uint32_t s0[32], s1[32];
+                    tmem_ld32(lane_base + b * 64, s0);
+                    tmem_ld32(lane_base + b * 64 + 32, s1);
+                    tmem_wait_ld();
+                    const int tok0 = (blk_begin + j * kChunkBlocks) * 16;
+                    const int nb = min(kChunkBlocks, nblk - j * kChunkBlocks);
+                    const int nvis = min(lim - tok0 + 1, nb * 16);   // visible columns (<= 0: none); stale columns masked too
+                    float x[64];
+#pragma unroll
+                    for (int k = 0; k < 32; ++k) {
+                        x[k] = __uint_as_float(s0[k]);
+                        x[32 + k] = __uint_as_float(s1[k]);
+                    }
+                    if (nvis < kChunk) {
+#pragma unroll
+                        for (int k = 0; k < 64; ++k)
+                            if (k >= nvis) x[k] = -INFINITY;
+                    }
+                    float mraw = x[0];
+#pragma unroll
+                    for (int k = 1; k < 63; k += 2) mraw = fmax3(mraw, x[k], x[k + 1]);
+                    mraw = fmaxf(mraw, x[63]);
+                    const float mx = mraw * p.scale_log2;   // -inf stays -inf
+                    bool need = false;
+                    float alpha = 1.f;
+                    if (j == 0) {
+                        m_used = mx;   // PV_0 overwrites O (accumulate = 0): nothing to rescale
+                    } else {
+                        need = mx > m_used + 8.f;   // lazy rescale: exponents stay below 2^8 otherwise
+                        if (need) {
+                            alpha = fast_exp2(m_used - mx);   // exp2(-inf) = 0 for a row with no key yet
+                            m_used = mx;
+                            l_run *= alpha;
+                        }
+                    }
+                    const float ref = m_used == -INFINITY ? 0.f : m_used;
+                    uint32_t pk[32];
+                    const float2 sc2 = make_float2(p.scale_log2, p.scale_log2), nref2 = make_float2(-ref, -ref);
+                    float2 acc2 = make_float2(0.f, 0.f);
+#pragma unroll
+                    for (int k = 0; k < 32; ++k) {
+                        const float2 tt = ffma2(make_float2(x[2 * k], x[2 * k + 1]), sc2, nref2);
+                        const float p0 = fast_exp2(tt.x), p1 = fast_exp2(tt.y);
+                        acc2 = fadd2(acc2, make_float2(p0, p1));
+                        pk[k] = pack_bf16(p0, p1);
+                    }
+                    l_run += acc2.x + acc2.y;
+                    if (j > 0) {
+                        mbar_wait(&o_done[t], (c - 1) & 1);   // PV_{j-1} of this tile has finished: O is stable
+                        tc_fence_after();
+                        if (__any_sync(0xffffffffu, need)) {
+#pragma unroll
+                            for (int piece = 0; piece < 4; ++piece) {
+                                uint32_t o[32];
+                                tmem_ld32(lane_base + 128 + piece * 32, o);
+                                tmem_wait_ld();
+#pragma unroll
+                                for (int k = 0; k < 32; ++k) o[k] = __float_as_uint(__uint_as_float(o[k]) * alpha);
+                                tmem_st32(lane_base + 128 + piece * 32, o);
+                            }
+                            tmem_wait_st();
+                        }
+                    }
+                    tmem_st32(lane_base + b * 64, pk);   // P_j over the first 32 columns of S_j (this lane's row only)
+                    tmem_wait_st();
+                    tc_fence_before();
+                    mbar_arrive(&p_full[t * 2 + b]);
+                }
+                // ---- epilogue: wait for this tile's last PV, normalise, write ----
+                mbar_wait(&o_done[t], (tc0 + nch - 1) & 1);
+                tc_fence_after();
+                const float inv = direct ? 1.f / l_run : 1.f;
+                const size_t orow = (size_t)(q_start + (ok ? sr / G : 0)) * p.Hq + (size_t)head * G + (ok ? sr % G : 0);
+                const size_t prow = (size_t)partial * 256 + t * 128 + r;
+#pragma unroll
+                for (int piece = 0; piece < 4; ++piece) {
+                    uint32_t o[32];
+                    tmem_ld32(lane_base + 128 + piece * 32, o);
+                    tmem_wait_ld();
+                    if (direct) {
+                        if (ok) {
+                            uint4* dst = reinterpret_cast<uint4*>(p.out + orow * D + piece * 32);
+#pragma unroll
+                            for (int q4 = 0; q4 < 4; ++q4) {
+                                uint4 w;
+                                w.x = pack_bf16(__uint_as_float(o[8 * q4 + 0]) * inv, __uint_as_float(o[8 * q4 + 1]) * inv);
+                                w.y = pack_bf16(__uint_as_float(o[8 * q4 + 2]) * inv, __uint_as_float(o[8 * q4 + 3]) * inv);
+                                w.z = pack_bf16(__uint_as_float(o[8 * q4 + 4]) * inv, __uint_as_float(o[8 * q4 + 5]) * inv);
+                                w.w = pack_bf16(__uint_as_float(o[8 * q4 + 6]) * inv, __uint_as_float(o[8 * q4 + 7]) * inv);
+                                dst[q4] = w;
+                            }
+                        }
+                    } else {
+                        uint4* dst = reinterpret_cast<uint4*>(p.po + prow * D + piece * 32);
+#pragma unroll
+                        for (int q4 = 0; q4 < 8; ++q4) dst[q4] = make_uint4(o[4 * q4], o[4 * q4 + 1], o[4 * q4 + 2], o[4 * q4 + 3]);
+                    }
+                }
+                if (direct) {
+                    if (ok) p.lse[orow] = (m_used + log2f(l_run)) * 0.6931471805599453f;
+                } else {
+                    *reinterpret_cast<float2*>(p.pml + prow * 2) = make_float2(m_used, l_run);
+                }
+            } else if (!direct) {
+                // tile B has no rows in this item: its partial slots must still read as "no key seen"
+                const size_t prow = (size_t)partial * 256 + 128 + (threadIdx.x & 127);
+                *reinterpret_cast<float2*>(p.pml + prow * 2) = make_float2(-INFINITY, 0.f);
+            }
+        }
+        kc += nch;
+        tcnA += nch;
+        if (hasB) tcnB += nch;
+        tc_fence_before();   // order this item's TMEM traffic before the next item's barrier
+    }
+    __syncthreads();
+    if (warp == 9) tmem_dealloc(tmem, kTmemCols2);
+}
+
+}   // namespace
+
+int launch_append_attn_tc2(const csv_plan* plan, const kv_pool* pool, int layer, const void* q, const int32_t* tables,
+                           int max_blocks, void* out, float* lse, void* stream) {
+    const kv_pool_desc& s = pool->desc;
+    AppendTc2Params p;
+    p.items = reinterpret_cast<const AppendItem*>(plan->d_ws + plan->lay.append_items);
+    p.n_items = (int32_t)plan->append_items.size();
+    p.pool_layer = pool->d_base + (size_t)layer * s.num_blocks * 2 * s.num_kv_heads * csv_tile_bytes(s.head_dim);
+    p.q = (const uint16_t*)q;
+    p.tables = tables;
+    p.out = (uint16_t*)out;
+    p.lse = lse;
+    p.po = reinterpret_cast<float*>(plan->d_ws + plan->lay.append_po);
+    p.pml = reinterpret_cast<float*>(plan->d_ws + plan->lay.append_pml);
+    p.max_blocks = max_blocks;
+    p.Hq = plan->shape.num_q_heads;
+    p.Hkv = plan->shape.num_kv_heads;
+    p.G = p.Hq / p.Hkv;
+    p.scale_log2 = (float)(1.4426950408889634 / sqrt((double)s.head_dim));
+    static bool attr_set = false;
+    if (!attr_set) {
+        CSV_CUDA_TRY(cudaFuncSetAttribute(append_tc2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes2));
+        attr_set = true;
+    }
+    const int grid = p.n_items < plan->num_sms ? p.n_items : plan->num_sms;
+    append_tc2_kernel<<<grid, kT2Threads, kSmemBytes2, (cudaStream_t)stream>>>(p);
+    CSV_CUDA_TRY(cudaGetLastError());
+    return CSV_OK;
+}

@@ -69,7 +69,7 @@ struct MergeGroup {
 
 constexpr int kDecodeWarps = 8;      // independent warp-workers per decode CTA
 constexpr int kAppendTileRows = 64;  // stacked rows per append work item of the mma.sync kernel (4 warps x 16)
-constexpr int kAppendTileRowsTc = 128;   // ... of the tcgen05 kernel (UMMA M)
+constexpr int kAppendTileRowsTc2 = 256;  // ... of the two-tile tcgen05 kernel (two UMMA M = 128 tiles sharing K/V)
 constexpr int kAppendKvSplit = 8192; // default KV tokens per append partition
 
 struct PlanLayout {   // byte offsets into the caller's workspace (all 128-byte aligned)
@@ -98,7 +98,7 @@ struct csv_plan {
     std::vector<AppendItem> append_items;
     std::vector<MergeGroup> append_groups;   // groups with count > 1 only
     int32_t n_append_chunks, n_append_rows;
-    int32_t append_tile_rows;                // stacked rows per append item: 128 (tcgen05, d = 128) or 64 (mma.sync, d = 64)
+    int32_t append_tile_rows;                // stacked rows per append item: 256 (tcgen05, d = 128: two UMMA tiles) or 64 (mma.sync, d = 64)
     int32_t n_append_partials;               // partial tiles (non-direct items)
     // device
     PlanLayout lay;
@@ -119,8 +119,8 @@ int launch_decode(const csv_plan* plan, const kv_pool* pool, int layer, const vo
                   const void* v_new = nullptr);
 int launch_append_attn(const csv_plan* plan, const kv_pool* pool, int layer, const void* q, const int32_t* tables,
                        int max_blocks, void* out, float* lse, void* stream);
-int launch_append_attn_tc(const csv_plan* plan, const kv_pool* pool, int layer, const void* q, const int32_t* tables,
-                          int max_blocks, void* out, float* lse, void* stream);
+int launch_append_attn_tc2(const csv_plan* plan, const kv_pool* pool, int layer, const void* q, const int32_t* tables,
+                           int max_blocks, void* out, float* lse, void* stream);
 int csv_query_num_sms();
 csv_plan* csv_plan_build_host(const csv_attn_shape* shape, const int32_t* h_q_lens, const int32_t* h_kv_lens,
                               int32_t batch, int32_t max_partition_tokens, int* err);

@@ -112,7 +112,7 @@ static void plan_decode(csv_plan* p) {
 static void plan_append(csv_plan* p) {
     const int Hkv = p->shape.num_kv_heads;
     const int G = p->shape.num_q_heads / Hkv;
-    const int TR = p->append_tile_rows = p->shape.head_dim == 128 ? kAppendTileRowsTc : kAppendTileRows;
+    const int TR = p->append_tile_rows = p->shape.head_dim == 128 ? kAppendTileRowsTc2 : kAppendTileRows;
     p->n_append_chunks = 0;
     p->n_append_rows = 0;
     p->append_items.clear();

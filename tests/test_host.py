@@ -246,15 +246,15 @@ def test_append_plan_covers_all_rows_and_visible_blocks():
         assert plan.total_q == q_start[-1]
         cover = {}
         for conv, head, r0, qs, m, kv_len, b0, b1, partial, direct, _, _ in items:
-            assert m == q_lens[conv] > 1 and kv_len == kv_lens[conv] and qs == q_start[conv] and r0 % 128 == 0
+            assert m == q_lens[conv] > 1 and kv_len == kv_lens[conv] and qs == q_start[conv] and r0 % 256 == 0
             cover.setdefault((conv, head, r0), []).append((b0, b1, direct))
         chunks = [b for b in range(len(q_lens)) if q_lens[b] > 1]
-        want = {(b, g, r0) for b in chunks for g in range(Hkv) for r0 in range(0, q_lens[b] * G, 128)}
+        want = {(b, g, r0) for b in chunks for g in range(Hkv) for r0 in range(0, q_lens[b] * G, 256)}
         assert set(cover) == want
         for (conv, head, r0), parts in cover.items():
             parts.sort()
             m, P = q_lens[conv], kv_lens[conv] - q_lens[conv]
-            i_max = min(m - 1, (min(m * G, r0 + 128) - 1) // G)   # d = 128: 128-row tiles (tcgen05 kernel)
+            i_max = min(m - 1, (min(m * G, r0 + 256) - 1) // G)   # d = 128: 256-row items (two 128-row UMMA tiles)
             assert parts[0][0] == 0 and parts[-1][1] == (P + i_max + 1 + 15) // 16   # exactly the visible blocks
             for (a0, a1, _), (c0, c1, _) in zip(parts, parts[1:]):
                 assert a1 == c0
