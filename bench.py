@@ -199,11 +199,17 @@ def handoff_extra(iters=5):
     payload = sum(toks) * NL * Hkv * d * 2 * 2                  # K + V bytes of all conversations
     pack_ms, _ = time_calls(lambda: B.kv_pack_batch(desc, ks, vs, toks, offs, sts), iters, 2)
     unpack_ms, _ = time_calls(lambda: B.kv_unpack_batch(pool, sts, toks, offs, ids, nids), iters, 2)
+    direct_ms, _ = time_calls(lambda: B.kv_handoff_direct_batch(pool, ks, vs, toks, offs, ids, nids), iters, 2)
     moved_unpack = sum(B.kv_staging_bytes(desc, t) for t in toks)   # whole tiles (last block padded)
     out = {"workload": "configs[3] c4_handoff_32layer", "tokens_total": sum(toks), "payload_gb": payload / 1e9,
            "pack_ms": pack_ms, "unpack_ms": unpack_ms,
            "pack_gbs_rw": 2 * payload / pack_ms / 1e6, "unpack_gbs_rw": 2 * payload / unpack_ms / 1e6,
-           "unpack_bytes_touched_gb": 2 * moved_unpack / 1e9}
+           "unpack_bytes_touched_gb": 2 * moved_unpack / 1e9,
+           # kv_handoff_direct: source -> paged pool in one kernel, no staging message (same GPU here; the
+           # destination may be a peer mapping).  Same payload, half the memory traffic of pack + unpack.
+           "direct_ms": direct_ms, "direct_gbs_rw": 2 * payload / direct_ms / 1e6,
+           "handoff_payload_gbs": {"pack_then_unpack": payload / (pack_ms + unpack_ms) / 1e6,
+                                   "direct": payload / direct_ms / 1e6}}
     del ks, vs, sts, d_pool
     torch.cuda.empty_cache()
     return out

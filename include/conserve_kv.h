@@ -196,6 +196,44 @@ int kv_unpack_batch(kv_pool_t* dst, int32_t n, const void* const* h_d_staging,
                     const int32_t* h_tokens, const int32_t* h_token_offsets,
                     const int32_t* const* h_d_block_ids, const int32_t* h_n_ids, void* stream);
 
+/* Direct one-shot handoff: the composition
+ * kv_unpack(kv_pack(.)) in ONE kernel with no staging message.
+ * §4: "the resulting KV cache is transferred once to the bound decoder";
+ * PAPER.md:96 §3.1 / Fig. 3: the transfer is the cost the handoff adds.  The
+ * kernel runs on the CURRENT device, which must be the one holding d_k / d_v
+ * (the prefiller), and pushes 16-byte stores into `dst`'s memory; dst's
+ * d_base may be local (two pools on one GPU) or a PEER mapping of the
+ * decoder's pool (csv_ipc_open below, or cudaDeviceEnablePeerAccess inside
+ * one process): the stores then cross NVLink and nothing is loaded from the
+ * peer.  d_k, d_v: [NL][tokens][Hkv][d] bf16, 16-byte aligned, as kv_pack.
+ * d_block_ids: the conversation's table as kv_unpack, readable on the current
+ * device (the router sends the ids with the binding: a few KB).  Result in the
+ * pool: bit-identical to kv_unpack(kv_pack(.)); slots not addressed are NOT
+ * written.  Ordering across GPUs is the caller's: the decoder may read the
+ * blocks after the prefiller's stream has passed this call (event / message). */
+int kv_handoff_direct(kv_pool_t* dst, const void* d_k, const void* d_v, int32_t tokens, int32_t token_offset,
+                      const int32_t* d_block_ids, int32_t n_ids, void* stream);
+int kv_handoff_direct_batch(kv_pool_t* dst, int32_t n, const void* const* h_d_k, const void* const* h_d_v,
+                            const int32_t* h_tokens, const int32_t* h_token_offsets,
+                            const int32_t* const* h_d_block_ids, const int32_t* h_n_ids, void* stream);
+
+/* Peer mapping for one process per GPU (CUDA IPC), so that a prefiller
+ * process can wrap a decoder process's pool memory in its own kv_pool_t
+ * (kv_pool_create over the opened pointer; the ALLOCATOR state stays with the
+ * decoder, which allocates the blocks and sends their ids).
+ * csv_ipc_export: d_ptr is any device pointer inside a cudaMalloc allocation
+ *   of the calling process; writes the CSV_IPC_HANDLE_BYTES-byte handle of the
+ *   allocation and d_ptr's byte offset inside it.  Host bytes, sendable over
+ *   any channel (torch.distributed object collectives in the tests).
+ * csv_ipc_open: in another process, maps the allocation (peer access enabled
+ *   lazily when it lives on another GPU) and returns base + offset.
+ * csv_ipc_close: unmaps; d_ptr is what csv_ipc_open returned.
+ * Errors: CSV_E_INVAL bad argument / unknown pointer, CSV_E_CUDA otherwise. */
+#define CSV_IPC_HANDLE_BYTES 64
+int csv_ipc_export(const void* d_ptr, void* out_handle, uint64_t* out_offset);
+int csv_ipc_open(const void* handle, uint64_t offset, void** out_d_ptr);
+int csv_ipc_close(void* d_ptr);
+
 /* Tail-step KV append ("appending one new entry"; PAPER.md:94
  * "only calculating new KV cache entries for the appended tokens"): writes the
  * new tokens' K/V of a whole batch straight from token-major projections into

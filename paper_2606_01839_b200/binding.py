@@ -23,8 +23,9 @@ SYMBOLS = [
     "kv_unpack", "kv_pack_batch", "kv_unpack_batch", "kv_append_tokens", "csv_plan_workspace_bytes",
     "csv_plan_create", "csv_plan_destroy", "csv_plan_info", "csv_plan_total_q", "csv_plan_decode_items",
     "csv_plan_append_items", "paged_decode_attn", "paged_decode_step", "append_prefill_attn", "csv_tail_step_host_workspace_bytes",
-    "csv_tail_step_host",
+    "csv_tail_step_host", "kv_handoff_direct", "kv_handoff_direct_batch", "csv_ipc_export", "csv_ipc_open", "csv_ipc_close",
 ]
+IPC_HANDLE_BYTES = 64
 
 
 class KvPoolDesc(ctypes.Structure):
@@ -79,6 +80,11 @@ def lib():
             "kv_pack_batch": (ctypes.c_int, [pdesc, i32, pvp, pvp, pi32, pi32, pvp, vp]),
             "kv_unpack_batch": (ctypes.c_int, [vp, i32, pvp, pi32, pi32, pvp, pi32, vp]),
             "kv_append_tokens": (ctypes.c_int, [vp, vp, vp, vp, vp, i32, vp]),
+            "kv_handoff_direct": (ctypes.c_int, [vp, vp, vp, i32, i32, vp, i32, vp]),
+            "kv_handoff_direct_batch": (ctypes.c_int, [vp, i32, pvp, pvp, pi32, pi32, pvp, pi32, vp]),
+            "csv_ipc_export": (ctypes.c_int, [vp, vp, ctypes.POINTER(ctypes.c_uint64)]),
+            "csv_ipc_open": (ctypes.c_int, [vp, ctypes.c_uint64, pvp]),
+            "csv_ipc_close": (ctypes.c_int, [vp]),
             "csv_plan_workspace_bytes": (sz, [pshape, pi32, pi32, i32, i32]),
             "csv_plan_create": (ctypes.c_int, [pshape, pi32, pi32, i32, i32, vp, sz, vp, pvp]),
             "csv_plan_destroy": (ctypes.c_int, [vp]),
@@ -258,6 +264,39 @@ def kv_unpack_batch(pool, d_stagings, tokens, token_offsets, d_block_ids, n_ids,
     _, pn = _i32(n_ids)
     _check("kv_unpack_batch", lib().kv_unpack_batch(pool.handle, n, _vparr(d_stagings), pt, po, _vparr(d_block_ids), pn,
                                                     _stream(stream)))
+
+
+def kv_handoff_direct(pool, d_k, d_v, tokens, token_offset, d_block_ids, n_ids, stream=None):
+    _check("kv_handoff_direct", lib().kv_handoff_direct(pool.handle, _ptr(d_k), _ptr(d_v), tokens, token_offset,
+                                                        _ptr(d_block_ids), n_ids, _stream(stream)))
+
+
+def kv_handoff_direct_batch(pool, d_ks, d_vs, tokens, token_offsets, d_block_ids, n_ids, stream=None):
+    n = len(d_ks)
+    _, pt = _i32(tokens)
+    _, po = _i32(token_offsets)
+    _, pn = _i32(n_ids)
+    _check("kv_handoff_direct_batch", lib().kv_handoff_direct_batch(pool.handle, n, _vparr(d_ks), _vparr(d_vs), pt, po,
+                                                                    _vparr(d_block_ids), pn, _stream(stream)))
+
+
+def csv_ipc_export(t):
+    """(handle bytes, offset) of the cudaMalloc allocation holding tensor / pointer t: plain host data for any channel."""
+    h = ctypes.create_string_buffer(IPC_HANDLE_BYTES)
+    off = ctypes.c_uint64()
+    _check("csv_ipc_export", lib().csv_ipc_export(_ptr(t), h, ctypes.byref(off)))
+    return bytes(h.raw), int(off.value)
+
+
+def csv_ipc_open(handle, offset):
+    """Maps another process's allocation; returns the device pointer (int) of base + offset."""
+    out = ctypes.c_void_p()
+    _check("csv_ipc_open", lib().csv_ipc_open(ctypes.c_char_p(handle), offset, ctypes.byref(out)))
+    return int(out.value)
+
+
+def csv_ipc_close(ptr):
+    _check("csv_ipc_close", lib().csv_ipc_close(ctypes.c_void_p(ptr)))
 
 
 def csv_plan_workspace_bytes(shape, q_lens, kv_lens, max_partition_tokens=0):

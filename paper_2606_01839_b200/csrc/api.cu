@@ -1,6 +1,9 @@
 // api.cu — the extern "C" entry points of include/conserve_kv.h that touch CUDA: argument
 // validation, plan upload, launches, and the host-buffer tail step.  No kernels here.
+#include <string.h>
+
 #include <new>
+#include <vector>
 
 #include "common.cuh"
 #include "internal.h"
@@ -81,6 +84,91 @@ int kv_unpack(kv_pool_t* dst, const void* d_staging, int32_t tokens, int32_t tok
               int32_t n_ids, void* stream) {
     if (tokens <= 0) return CSV_E_INVAL;
     return kv_unpack_batch(dst, 1, &d_staging, &tokens, &token_offset, &d_block_ids, &n_ids, stream);
+}
+
+int kv_handoff_direct_batch(kv_pool_t* dst, int32_t n, const void* const* h_d_k, const void* const* h_d_v,
+                            const int32_t* h_tokens, const int32_t* h_token_offsets,
+                            const int32_t* const* h_d_block_ids, const int32_t* h_n_ids, void* stream) {
+    if (!dst || n < 0) return CSV_E_INVAL;
+    if (n > 0 && (!h_d_k || !h_d_v || !h_tokens || !h_token_offsets || !h_d_block_ids || !h_n_ids)) return CSV_E_INVAL;
+    for (int i = 0; i < n; ++i) {
+        if (h_tokens[i] < 0 || h_token_offsets[i] < 0) return CSV_E_INVAL;
+        if (h_tokens[i] == 0) continue;
+        if (!h_d_k[i] || !h_d_v[i] || !h_d_block_ids[i]) return CSV_E_INVAL;
+        if (!aligned(h_d_k[i], 16) || !aligned(h_d_v[i], 16) || !aligned(h_d_block_ids[i], 4)) return CSV_E_INVAL;
+        const int64_t need = ((int64_t)h_token_offsets[i] + h_tokens[i] + 15) / 16;
+        if ((int64_t)h_n_ids[i] < need) return CSV_E_INVAL;
+    }
+    return launch_handoff_direct(dst, n, h_d_k, h_d_v, h_tokens, h_token_offsets, h_d_block_ids, stream);
+}
+
+int kv_handoff_direct(kv_pool_t* dst, const void* d_k, const void* d_v, int32_t tokens, int32_t token_offset,
+                      const int32_t* d_block_ids, int32_t n_ids, void* stream) {
+    if (tokens <= 0) return CSV_E_INVAL;
+    return kv_handoff_direct_batch(dst, 1, &d_k, &d_v, &tokens, &token_offset, &d_block_ids, &n_ids, stream);
+}
+
+// ---- peer mapping of a decoder's pool (one process per GPU: CUDA IPC) ----
+// cuMemGetAddressRange comes from the driver through the runtime's entry-point query: the library links no libcuda.
+typedef int (*cu_get_range_fn)(unsigned long long*, size_t*, unsigned long long);
+
+static cu_get_range_fn driver_get_range() {
+    static cu_get_range_fn fn = nullptr;
+    if (!fn) {
+        void* f = nullptr;
+        cudaDriverEntryPointQueryResult st;
+        if (cudaGetDriverEntryPoint("cuMemGetAddressRange", &f, cudaEnableDefault, &st) == cudaSuccess &&
+            st == cudaDriverEntryPointSuccess)
+            fn = (cu_get_range_fn)f;
+    }
+    return fn;
+}
+
+struct ipc_mapping {
+    void* user;   // what csv_ipc_open returned
+    void* base;   // what cudaIpcOpenMemHandle returned
+};
+static std::vector<ipc_mapping> g_ipc;   // host calls are thread-compatible, not thread-safe (header)
+
+int csv_ipc_export(const void* d_ptr, void* out_handle, uint64_t* out_offset) {
+    if (!d_ptr || !out_handle || !out_offset) return CSV_E_INVAL;
+    static_assert(sizeof(cudaIpcMemHandle_t) == CSV_IPC_HANDLE_BYTES, "handle size");
+    cu_get_range_fn get_range = driver_get_range();
+    if (!get_range) return csv_set_cuda_error((int)cudaErrorNotSupported);
+    unsigned long long base = 0;
+    size_t size = 0;
+    if (get_range(&base, &size, (unsigned long long)(uintptr_t)d_ptr) != 0) return csv_set_cuda_error((int)cudaErrorInvalidValue);
+    cudaIpcMemHandle_t h;
+    CSV_CUDA_TRY(cudaIpcGetMemHandle(&h, (void*)(uintptr_t)base));
+    memcpy(out_handle, &h, sizeof(h));
+    *out_offset = (uint64_t)((uintptr_t)d_ptr - (uintptr_t)base);
+    return CSV_OK;
+}
+
+int csv_ipc_open(const void* handle, uint64_t offset, void** out_d_ptr) {
+    if (!handle || !out_d_ptr) return CSV_E_INVAL;
+    cudaIpcMemHandle_t h;
+    memcpy(&h, handle, sizeof(h));
+    void* base = nullptr;
+    CSV_CUDA_TRY(cudaIpcOpenMemHandle(&base, h, cudaIpcMemLazyEnablePeerAccess));
+    ipc_mapping m;
+    m.base = base;
+    m.user = (uint8_t*)base + offset;
+    g_ipc.push_back(m);
+    *out_d_ptr = m.user;
+    return CSV_OK;
+}
+
+int csv_ipc_close(void* d_ptr) {
+    for (size_t i = 0; i < g_ipc.size(); ++i) {
+        if (g_ipc[i].user == d_ptr) {
+            void* base = g_ipc[i].base;
+            g_ipc.erase(g_ipc.begin() + (long)i);
+            CSV_CUDA_TRY(cudaIpcCloseMemHandle(base));
+            return CSV_OK;
+        }
+    }
+    return CSV_E_INVAL;
 }
 
 // Points a host-built plan at its device workspace and enqueues the upload of its work lists.

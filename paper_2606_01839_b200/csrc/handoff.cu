@@ -1,4 +1,4 @@
-// handoff.cu — kv_pack / kv_unpack / kv_append_tokens: the one-shot KV handoff (a2, a3;
+// handoff.cu — kv_pack / kv_unpack / kv_handoff_direct / kv_append_tokens: the one-shot KV handoff (a2, a3;
 // PAPER.md:150 §4 "transferred once", §3.1 cost linear in tokens) and the
 // tail step's new-token KV write (§2.1 "appending one new entry").
 //
@@ -42,6 +42,19 @@ struct UnpackParams {
     int32_t n, total_units, NL, Hkv;
     int32_t num_blocks, pad;
     uint8_t* pool;
+};
+
+struct DirectEntry {
+    const uint8_t* k;
+    const uint8_t* v;
+    const int32_t* ids;     // conversation's table, readable on the device that runs the kernel
+    int32_t tokens, slot0, ntb, blk0, unit_begin, pad;
+};
+struct DirectParams {
+    DirectEntry e[kMaxBatch];
+    int32_t n, total_units, NL, Hkv;
+    int32_t num_blocks, pad;
+    uint8_t* pool;          // local or peer-mapped (NVLink) pool base
 };
 
 // Plain ld / st: measured faster here than .nc / L1::no_allocate / .cs hints (6.8 vs 6.2 TB/s).
@@ -134,6 +147,55 @@ __global__ void __launch_bounds__(kThreads, 4) unpack_kernel(const __grid_consta
 #pragma unroll
             for (int j = 0; j < U; ++j)
                 if (ok[j]) st16(dst + (size_t)(c0 + j * kThreads) * 16, val[j]);
+        }
+    }
+}
+
+// kv_handoff_direct: pack and unpack composed, no staging message ("transferred once to
+// the bound decoder").  Unit = (conversation, layer, block, K|V): 16 contiguous source token rows (32 KiB at the 8B
+// shape) -> the Hkv tiles of (layer, table[block], K|V), also 32 KiB contiguous in the destination pool.  The kernel runs
+// where the source lives and PUSHES: loads are local and coalesced, stores are whole 128-byte tile rows and may cross
+// NVLink (posted writes; nothing is ever loaded from the peer).  Slots outside the message are not written.
+template <int D, int U>
+__global__ void __launch_bounds__(kThreads, 4) direct_kernel(const __grid_constant__ DirectParams p) {
+    constexpr int CPR = D / 8;
+    constexpr int LCPR = D == 128 ? 4 : 3;
+    constexpr int TB = 16 * D * 2;
+    const int lh = 31 - __clz(p.Hkv);
+    const int chunks_per_unit = 16 * p.Hkv * CPR;
+    const size_t row_bytes = (size_t)p.Hkv * D * 2;
+    for (int unit = blockIdx.x; unit < p.total_units; unit += gridDim.x) {
+        const int ei = find_entry(p, unit);
+        const DirectEntry& e = p.e[ei];
+        const int u = unit - e.unit_begin;      // ((layer * ntb) + tb) * 2 + kv
+        const int kv = u & 1;
+        const int layer = (u >> 1) / e.ntb;
+        const int tb = (u >> 1) - layer * e.ntb;
+        const int block = __ldg(e.ids + e.blk0 + tb);
+        const uint8_t* src_layer = (kv ? e.v : e.k) + (size_t)layer * e.tokens * row_bytes;
+        uint8_t* dst_unit = p.pool + (((size_t)layer * p.num_blocks + block) * 2 + kv) * p.Hkv * TB;
+        const int tok_base = tb * 16 - e.slot0;
+        const uint8_t* src_row0 = src_layer + (ptrdiff_t)tok_base * (ptrdiff_t)row_bytes;
+        for (int c0 = threadIdx.x; c0 < chunks_per_unit; c0 += kThreads * U) {
+            uint4 val[U];
+            bool ok[U];
+#pragma unroll
+            for (int j = 0; j < U; ++j) {
+                const int c = c0 + j * kThreads;
+                const int tok = tok_base + (c >> (LCPR + lh));
+                ok[j] = c < chunks_per_unit && tok >= 0 && tok < e.tokens;
+                if (ok[j]) val[j] = ld16(src_row0 + (size_t)c * 16);
+            }
+#pragma unroll
+            for (int j = 0; j < U; ++j) {
+                if (ok[j]) {
+                    const int c = c0 + j * kThreads;
+                    const int chunk = c & (CPR - 1);
+                    const int head = (c >> LCPR) & (p.Hkv - 1);
+                    const int slot = c >> (LCPR + lh);
+                    st16(dst_unit + head * TB + (chunk >> 3) * 2048 + slot * 128 + (((chunk & 7) ^ (slot & 7)) << 4), val[j]);
+                }
+            }
         }
     }
 }
@@ -264,6 +326,52 @@ int launch_unpack(kv_pool* dst, int n, const void* const* staging, const int32_t
             unpack_kernel<128, 8><<<grid, kThreads, 0, (cudaStream_t)stream>>>(p);
         } else {
             unpack_kernel<64, 4><<<grid, kThreads, 0, (cudaStream_t)stream>>>(p);
+        }
+        CSV_CUDA_TRY(cudaGetLastError());
+    }
+    return CSV_OK;
+}
+
+int launch_handoff_direct(kv_pool* dst, int n, const void* const* k, const void* const* v, const int32_t* tokens,
+                          const int32_t* offs, const int32_t* const* block_ids, void* stream) {
+    const kv_pool_desc& shape = dst->desc;
+    int i = 0;
+    while (i < n) {
+        DirectParams p;
+        p.n = 0;
+        p.NL = shape.num_layers;
+        p.Hkv = shape.num_kv_heads;
+        p.num_blocks = shape.num_blocks;
+        p.pool = dst->d_base;
+        long long units = 0;
+        while (i < n && p.n < kMaxBatch) {
+            if (tokens[i] > 0) {
+                DirectEntry& e = p.e[p.n];
+                e.k = (const uint8_t*)k[i];
+                e.v = (const uint8_t*)v[i];
+                e.ids = block_ids[i];
+                e.tokens = tokens[i];
+                e.slot0 = offs[i] & 15;
+                e.ntb = (e.slot0 + e.tokens + 15) / 16;
+                e.blk0 = offs[i] >> 4;
+                const long long nu = (long long)shape.num_layers * e.ntb * 2;
+                if (units + nu > INT32_MAX) break;
+                e.unit_begin = (int32_t)units;
+                units += nu;
+                ++p.n;
+            }
+            ++i;
+        }
+        if (p.n == 0) {
+            if (i < n && tokens[i] > 0) return CSV_E_INVAL;
+            continue;
+        }
+        p.total_units = (int32_t)units;
+        const int grid = grid_for(p.total_units);
+        if (shape.head_dim == 128) {
+            direct_kernel<128, 4><<<grid, kThreads, 0, (cudaStream_t)stream>>>(p);
+        } else {
+            direct_kernel<64, 4><<<grid, kThreads, 0, (cudaStream_t)stream>>>(p);
         }
         CSV_CUDA_TRY(cudaGetLastError());
     }

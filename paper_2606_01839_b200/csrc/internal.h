@@ -110,6 +110,8 @@ struct csv_plan {
 int csv_set_cuda_error(int err);   // records err, returns CSV_E_CUDA
 int launch_pack(const kv_pool_desc& shape, int n, const void* const* k, const void* const* v, const int32_t* tokens,
                 const int32_t* offs, void* const* staging, void* stream);
+int launch_handoff_direct(kv_pool* dst, int n, const void* const* k, const void* const* v, const int32_t* tokens,
+                          const int32_t* offs, const int32_t* const* block_ids, void* stream);
 int launch_unpack(kv_pool* dst, int n, const void* const* staging, const int32_t* tokens, const int32_t* offs,
                   const int32_t* const* block_ids, void* stream);
 int launch_append_tokens(kv_pool* dst, const csv_plan* plan, const void* k_new, const void* v_new,

@@ -1,5 +1,5 @@
 """Small driver for ncu captures of the kernels bench.py does not put first (profiles/*.md name the commands):
-  python -m paper_2606_01839_b200.profile_cases handoff   one kv_pack + kv_unpack of a 32-layer, 16384-token conversation
+  python -m paper_2606_01839_b200.profile_cases handoff   one kv_pack + kv_unpack + kv_handoff_direct of a 32-layer, 16384-token conversation
   python -m paper_2606_01839_b200.profile_cases tail      config 3 (agentic tail mix): paged_decode_attn + append_prefill_attn
 Three calls each; inputs are the same seeded synthetic ones the tests and bench use."""
 import sys
@@ -24,6 +24,7 @@ if what == "handoff":
     for _ in range(3):
         B.kv_pack(desc, k, v, t, 0, st)
         B.kv_unpack(pool, st, t, 0, ids, len(ids))
+        B.kv_handoff_direct(pool, k, v, t, 0, ids, len(ids))
     torch.cuda.synchronize()
 else:
     wl = workloads.config_tail_workload(3)

@@ -41,3 +41,83 @@ def aggregate(dist, local_ms, local_units, device="cpu"):
     dist.all_reduce(t, op=dist.ReduceOp.MAX)
     dist.all_reduce(u, op=dist.ReduceOp.SUM)
     return float(t.item()), float(u.item())
+
+
+# ---------------- cross-GPU one-shot handoff ("transferred once to the bound decoder") ------
+# Protocol, one process per GPU:  the DECODER owns its pool and allocator; it allocates the conversation's blocks and
+# sends a ticket (plain host data: shape, block ids, the IPC handle of the pool's allocation).  The PREFILLER maps the
+# pool once per decoder, wraps it in a kv_pool_t and pushes the conversation with kv_handoff_direct: its stores cross
+# NVLink, nothing is staged or loaded from the peer.  It then tells the decoder (any message after a stream sync).
+
+def handoff_ticket(pool, tokens, token_offset=0, ids=None, export=None, decoder=0):
+    """Decoder side.  pool: binding.KvPool.  Allocates ceil((offset + tokens) / 16) blocks unless the conversation's
+    table `ids` is given (a later push into blocks it already owns).  export: (handle, offset) from
+    binding.csv_ipc_export(pool memory), or None when prefiller and decoder share a process.  All-or-nothing."""
+    from . import binding as B
+
+    if tokens <= 0 or token_offset < 0:
+        raise ValueError("tokens must be > 0 and token_offset >= 0")
+    need = (token_offset + tokens + B.BLOCK - 1) // B.BLOCK
+    if ids is None:
+        ids = pool.alloc_blocks(need)                      # raises CsvError(CSV_E_NOMEM) and changes nothing if short
+    if len(ids) < need:
+        raise ValueError("table shorter than ceil((offset + tokens) / 16)")
+    d = pool.desc
+    return {"decoder": int(decoder), "tokens": int(tokens), "token_offset": int(token_offset),
+            "ids": [int(i) for i in ids],
+            "shape": (int(d.num_layers), int(d.num_blocks), int(d.num_kv_heads), int(d.head_dim)),
+            "handle": None if export is None else bytes(export[0]), "offset": 0 if export is None else int(export[1])}
+
+
+def send_ticket(dist, ticket, dst):
+    dist.send_object_list([ticket], dst=dst)
+
+
+def recv_ticket(dist, src):
+    box = [None]
+    dist.recv_object_list(box, src=src)
+    return box[0]
+
+
+class PeerPools:
+    """Prefiller side: one mapping + kv_pool_t wrapper per decoder pool, opened on first use."""
+
+    def __init__(self):
+        self._pools = {}
+
+    def get(self, ticket, local_pool=None):
+        from . import binding as B
+
+        key = (ticket["decoder"], ticket["handle"], ticket["offset"])
+        if key not in self._pools:
+            NL, nb, Hkv, d = ticket["shape"]
+            desc = B.pool_desc(NL, nb, Hkv, d)
+            if ticket["handle"] is None:
+                if local_pool is None:
+                    raise ValueError("ticket without an IPC handle needs the local pool")
+                self._pools[key] = (local_pool, None)
+            else:
+                ptr = B.csv_ipc_open(ticket["handle"], ticket["offset"])
+                self._pools[key] = (B.KvPool(desc, ptr, B.kv_pool_bytes(desc)), ptr)
+        return self._pools[key][0]
+
+    def push(self, ticket, d_k, d_v, d_ids=None, stream=None, local_pool=None):
+        """kv_handoff_direct of one conversation into the ticket's pool.  d_k, d_v: [NL][tokens][Hkv][d] bf16 device
+        tensors of THIS process.  Returns the device id tensor used (keep it alive until the stream has passed)."""
+        import torch
+        from . import binding as B
+
+        pool = self.get(ticket, local_pool)
+        if d_ids is None:
+            d_ids = torch.tensor(ticket["ids"], dtype=torch.int32, device="cuda")
+        B.kv_handoff_direct(pool, d_k, d_v, ticket["tokens"], ticket["token_offset"], d_ids, len(ticket["ids"]), stream)
+        return d_ids
+
+    def close(self):
+        from . import binding as B
+
+        for pool, ptr in self._pools.values():
+            if ptr is not None:
+                pool.destroy()
+                B.csv_ipc_close(ptr)
+        self._pools = {}

@@ -50,3 +50,56 @@ def test_placement_replay_balances_decoders():
     got = replicas.bind_conversations(need, pool_blocks=60, world=2)
     assert got == [0, 1, 0, 1, 0, 0, -1, 0]
     assert replicas.aggregate(None, 1.5, 7.0) == (1.5, 7.0)
+
+
+FAKE = 1 << 40          # a 128-byte aligned "device" address: the allocator and tickets are host-only
+
+
+def _handoff_worker(rank, world, port, ret):
+    """rank 0 = prefiller, ranks 1.. = decoders.  Host side of the cross-GPU handoff: the router's
+    placement (csv_place), block allocation on the bound decoder, the ticket's trip to the prefiller."""
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    desc = B.pool_desc(2, 64, 8, 128)
+    if rank == 0:
+        got = [replicas.recv_ticket(dist, 1) for _ in range(3)]
+        ret[0] = got
+    else:
+        pool = B.KvPool(desc, FAKE, B.kv_pool_bytes(desc))
+        pool.set_free_order(np.arange(63, -1, -1))
+        export = (bytes(range(64)), 8192)                  # stands in for csv_ipc_export (needs a GPU)
+        t1 = replicas.handoff_ticket(pool, 300, export=export, decoder=1)
+        t2 = replicas.handoff_ticket(pool, 5, 11, export=export, decoder=1)
+        t3 = replicas.handoff_ticket(pool, 20, 300, ids=t1["ids"] + list(pool.alloc_blocks(1)), export=export, decoder=1)
+        for t in (t1, t2, t3):
+            replicas.send_ticket(dist, t, 0)
+        try:
+            replicas.handoff_ticket(pool, 16 * 64)         # more than the pool has left: all-or-nothing
+            full = False
+        except B.CsvError as e:
+            full = e.code == B.CSV_E_NOMEM
+        ret[1] = (pool.used_blocks, full)
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_handoff_tickets_travel_from_decoder_to_prefiller():
+    libbuild.build_library()
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    mgr = mp.get_context("spawn").Manager()
+    ret = mgr.dict()
+    mp.spawn(_handoff_worker, args=(2, port, ret), nprocs=2, join=True)
+    t1, t2, t3 = ret[0]
+    assert t1["ids"] == list(range(63, 44, -1)) and t1["tokens"] == 300 and t1["token_offset"] == 0   # 19 blocks, free order
+    assert t2["ids"] == [44] and t2["token_offset"] == 11
+    assert t3["ids"] == t1["ids"] + [43] and t3["token_offset"] == 300
+    assert t1["shape"] == (2, 64, 8, 128) and t1["handle"] == bytes(range(64)) and t1["offset"] == 8192
+    assert ret[1] == (21, True)                            # occupancy the placement rule reads; the failed ticket took nothing
+    pools = replicas.PeerPools()
+    try:
+        pools.get({"decoder": 0, "handle": None, "offset": 0, "shape": (1, 1, 1, 64)})
+        assert False
+    except ValueError:
+        pass
