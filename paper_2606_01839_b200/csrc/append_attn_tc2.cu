@@ -9,8 +9,8 @@
 // between the two tiles while the other tile's softmax runs.
 //   warps 0-3  softmax of tile A, warps 4-7 softmax of tile B (thread r owns row r = TMEM lane r % 128)
 //   warp 8     producer: 1-D bulk copies of K half-tiles / V tiles into the rings
-//   warps 9,10 MMA issuers, one per tile (a single issuing thread needs ~90 cycles per tcgen05.mma, measured: it was
-//              the bottleneck with 24 MMAs per chunk): S_t = Q_t K^T (SS, M=128, N=64), O_t += P_t V (A = P from TMEM)
+//   warps 9,10 MMA issuers, one per tile (one issuer for both tiles serialises their dependent chains: measured 563
+//              against 957 TFLOP/s): S_t = Q_t K^T (SS, M=128, N=64), O_t += P_t V (A = P from TMEM)
 // TMEM (all 512 columns): tile t at t*256: S/P buffer 0 [0,64), buffer 1 [64,128), O [128,256).
 #include <math.h>
 
@@ -160,23 +160,32 @@ __global__ void __launch_bounds__(kT2Threads, 1) append_tc2_kernel(const __grid_
             const int t = warp - 9;
             const bool active = t == 0 || hasB;      // an idle issuer still releases the K/V stages
             const uint32_t tc0 = t ? tcnB : tcnA;
+            // descriptors are built once; per MMA only (byte offset >> 4) is added to the low word (tc5.cuh)
+            const uint64_t qd = smem_desc_sw128(sbase + kOffQ2 + t * 32768, 16, 1024);
+            const uint64_t kd = smem_desc_sw128(sbase + kOffK2, 16, 1024);
+            const uint64_t vd = smem_desc_sw128(sbase + kOffV2, 2048, 1024);
+            // broadcast through a shuffle: tells the compiler these are warp-uniform, so the per-MMA descriptor words are
+            // formed on the uniform datapath instead of one R2UR chain per MMA (measured: ~114 -> ~50-64 cycles per MMA)
+            const uint32_t q_lo = __shfl_sync(0xffffffffu, (uint32_t)qd, 0), qk_hi = __shfl_sync(0xffffffffu, (uint32_t)(qd >> 32), 0);
+            const uint32_t k_lo = __shfl_sync(0xffffffffu, (uint32_t)kd, 0);
+            const uint32_t v_lo = __shfl_sync(0xffffffffu, (uint32_t)vd, 0), v_hi = __shfl_sync(0xffffffffu, (uint32_t)(vd >> 32), 0);
+            const uint32_t tm_t = __shfl_sync(0xffffffffu, tmem + t * 256, 0);
+            const bool leader = lane == 0;
             auto issue_S = [&](int j) {
                 const uint32_t c = kc + j, ks = c % kKSt, kph = (c / kKSt) & 1;
                 mbar_wait(&k_full[ks], kph);
                 tc_fence_after();
-                {
+                const uint32_t bt = __shfl_sync(0xffffffffu, (tc0 + j) & 1, 0);
+                const uint32_t dS = tm_t + bt * 64, kl = k_lo + __shfl_sync(0xffffffffu, ks, 0) * 1024;
+                if (leader) {
                     if (active) {
-                        const uint32_t bt = (tc0 + j) & 1;
 #pragma unroll
-                        for (int hk = 0; hk < 8; ++hk) {   // hk = half * 4 + k-step inside the 64-element half
-                            const uint32_t off = (hk >> 2) * 16384 + (hk & 3) * 32;
-                            const uint32_t offk = (hk >> 2) * 8192 + (hk & 3) * 32;
-                            mma_ss_elect(tmem + t * 256 + bt * 64, smem_desc_sw128(sbase + kOffQ2 + t * 32768 + off, 16, 1024),
-                                   smem_desc_sw128(sbase + kOffK2 + ks * 16384 + offk, 16, 1024), idS, hk != 0);
-                        }
-                        tc_commit_elect(&s_full[t * 2 + bt]);
+                        for (int hk = 0; hk < 8; ++hk)   // hk = half * 4 + k-step inside the 64-element half
+                            mma_ss_lohi(dS, q_lo + (hk >> 2) * 1024 + (hk & 3) * 2, qk_hi, kl + (hk >> 2) * 512 + (hk & 3) * 2,
+                                        qk_hi, idS, hk != 0);
+                        tc_commit(&s_full[t * 2 + bt]);
                     }
-                    tc_commit_elect(&k_empty[ks]);
+                    tc_commit(&k_empty[ks]);
                 }
                 __syncwarp();
             };
@@ -199,14 +208,16 @@ __global__ void __launch_bounds__(kT2Threads, 1) append_tc2_kernel(const __grid_
                     __syncwarp();
                 }
                 tc_fence_after();
-                {
+                const uint32_t dO = tm_t + 128, aP = tm_t + __shfl_sync(0xffffffffu, bt, 0) * 64;
+                const uint32_t vl = v_lo + __shfl_sync(0xffffffffu, vs, 0) * 1024;
+                if (leader) {
                     if (active) {
-                        for (int kk = 0; kk < nb; ++kk)
-                            mma_ts_elect(tmem + t * 256 + 128, tmem + t * 256 + bt * 64 + kk * 8,
-                                   smem_desc_sw128(sbase + kOffV2 + vs * 16384 + kk * TB, 2048, 1024), idO, (j | kk) != 0);
-                        tc_commit_elect(&o_done[t]);
+#pragma unroll
+                        for (int kk = 0; kk < kChunkBlocks; ++kk)
+                            if (kk < nb) mma_ts_lohi(dO, aP + kk * 8, vl + kk * (TB >> 4), v_hi, idO, (j | kk) != 0);
+                        tc_commit(&o_done[t]);
                     }
-                    tc_commit_elect(&v_empty[vs]);
+                    tc_commit(&v_empty[vs]);
                 }
                 __syncwarp();
             }
@@ -260,6 +271,16 @@ __global__ void __launch_bounds__(kT2Threads, 1) append_tc2_kernel(const __grid_
                         }
                     }
                     const float ref = m_used == -INFINITY ? 0.f : m_used;
+                    // The XU (ex2) pipe of an SM sub-partition is shared by warp w (tile A) and warp w + 4 (tile B).  Left
+                    // alone the two drift into running their exponential phases together at half rate each; a token
+                    // passed between the pair makes them alternate (A first in every chunk).
+                    if (hasB) {
+                        if (t == 0) {
+                            if (j > 0) asm volatile("bar.sync %0, 64;" ::"r"(1 + (warp & 3)) : "memory");
+                        } else {
+                            asm volatile("bar.sync %0, 64;" ::"r"(5 + (warp & 3)) : "memory");
+                        }
+                    }
                     uint32_t pk[32];
                     const float2 sc2 = make_float2(p.scale_log2, p.scale_log2), nref2 = make_float2(-ref, -ref);
                     float2 acc2 = make_float2(0.f, 0.f);
@@ -271,6 +292,13 @@ __global__ void __launch_bounds__(kT2Threads, 1) append_tc2_kernel(const __grid_
                         pk[k] = pack_bf16(p0, p1);
                     }
                     l_run += acc2.x + acc2.y;
+                    if (hasB) {
+                        if (t == 0) {
+                            asm volatile("bar.arrive %0, 64;" ::"r"(5 + (warp & 3)) : "memory");
+                        } else if (j + 1 < nch) {
+                            asm volatile("bar.arrive %0, 64;" ::"r"(1 + (warp & 3)) : "memory");
+                        }
+                    }
                     if (j > 0) {
                         mbar_wait(&o_done[t], (c - 1) & 1);   // PV_{j-1} of this tile has finished: O is stable
                         tc_fence_after();

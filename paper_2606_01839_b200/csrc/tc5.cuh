@@ -64,26 +64,26 @@ __device__ __forceinline__ void mma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_
         : "memory");
 }
 
-// Warp-converged forms: every lane executes the call, one elected lane issues (no divergent region around the
-// MMA, so the descriptor arithmetic stays on the uniform datapath).
-__device__ __forceinline__ void mma_ss_elect(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
+// Single-thread forms taking the descriptor as (lo, hi) words: the caller builds the descriptor once and adds
+// (byte offset >> 4) to the low word per MMA (the start-address field is its low 14 bits).  With the base words made
+// warp-uniform (a shuffle broadcast tells the compiler) the per-MMA words are formed by UIADD3 on the uniform datapath.
+// Microbenchmark, one warp issuing back to back, nothing else on the SM: rebuilding the 64-bit descriptor and electing
+// per MMA costs ~115 cycles per MMA whatever the shape; this form runs at the pipe's rate: 48 cycles for M128 N64 K16
+// SS (6 KiB of shared-memory operands at 128 B/clk; the math is 32), 64 for N128 SS and N128 TS, 128 for N256 SS.
+__device__ __forceinline__ void mma_ss_lohi(uint32_t d_tmem, uint32_t a_lo, uint32_t a_hi, uint32_t b_lo, uint32_t b_hi,
+                                            uint32_t idesc, uint32_t accumulate) {
     asm volatile(
-        "{\n\t.reg .pred pe, pa;\n\telect.sync _|pe, 0xffffffff;\n\tsetp.ne.b32 pa, %4, 0;\n\t"
-        "@pe tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, pa;\n\t}"
-        ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)
+        "{\n\t.reg .pred pa;\n\t.reg .b64 da, db;\n\tsetp.ne.b32 pa, %6, 0;\n\tmov.b64 da, {%1, %2};\n\t"
+        "mov.b64 db, {%3, %4};\n\ttcgen05.mma.cta_group::1.kind::f16 [%0], da, db, %5, pa;\n\t}"
+        ::"r"(d_tmem), "r"(a_lo), "r"(a_hi), "r"(b_lo), "r"(b_hi), "r"(idesc), "r"(accumulate)
         : "memory");
 }
-__device__ __forceinline__ void mma_ts_elect(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
+__device__ __forceinline__ void mma_ts_lohi(uint32_t d_tmem, uint32_t a_tmem, uint32_t b_lo, uint32_t b_hi, uint32_t idesc,
+                                            uint32_t accumulate) {
     asm volatile(
-        "{\n\t.reg .pred pe, pa;\n\telect.sync _|pe, 0xffffffff;\n\tsetp.ne.b32 pa, %4, 0;\n\t"
-        "@pe tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, pa;\n\t}"
-        ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate)
-        : "memory");
-}
-__device__ __forceinline__ void tc_commit_elect(uint64_t* bar) {
-    asm volatile(
-        "{\n\t.reg .pred pe;\n\telect.sync _|pe, 0xffffffff;\n\t"
-        "@pe tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n\t}" ::"r"(smem_u32(bar))
+        "{\n\t.reg .pred pa;\n\t.reg .b64 db;\n\tsetp.ne.b32 pa, %5, 0;\n\tmov.b64 db, {%2, %3};\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], db, %4, pa;\n\t}"
+        ::"r"(d_tmem), "r"(a_tmem), "r"(b_lo), "r"(b_hi), "r"(idesc), "r"(accumulate)
         : "memory");
 }
 
