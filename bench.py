@@ -263,9 +263,18 @@ def tail_extra(k, iters=10):
         torch.cuda.current_stream().wait_stream(s1)
         torch.cuda.current_stream().wait_stream(s2)
 
-    if k == 5 or True:
-        both_ms, _ = time_calls(both, max(3, iters // 2))
-        out.update(decode_plus_append_overlapped_ms=both_ms)
+    both_ms, _ = time_calls(both, max(3, iters // 2))
+    out.update(decode_plus_append_overlapped_ms=both_ms)
+    if k == 3:
+        # the whole mixed step in one call (csv_tail_step: KV write of all 9347 new rows + decode + append), replayed
+        # from a CUDA graph as a serving loop would
+        g = torch.cuda.CUDAGraph()
+        wl.tail_step()
+        torch.cuda.synchronize()
+        with torch.cuda.graph(g):
+            wl.tail_step()
+        step_ms, _ = time_calls(g.replay, max(3, iters // 2))
+        out.update(tail_step_one_call_ms=step_ms)
     del wl, app
     torch.cuda.empty_cache()
     return out

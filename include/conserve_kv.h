@@ -342,6 +342,20 @@ int append_prefill_attn(const csv_plan_t* plan, const kv_pool_t* pool, int32_t l
                         const int32_t* d_block_tables, int32_t max_blocks, void* d_out, float* d_lse,
                         void* stream);
 
+/* One tail step of a MIXED batch on one layer (PAPER.md:112 /
+ * Fig. 5: decode rows and appended chunks run in the same iteration on the
+ * decoder that holds their prefixes): writes every new row's K/V into the
+ * pool, then attends.  Equivalent to kv_append_tokens (on this layer) +
+ * paged_decode_attn + append_prefill_attn, enqueued back to back on `stream`
+ * (programmatic dependent launch between the KV write and the decode); with no
+ * appended chunk in the plan it is paged_decode_step (KV write inside the
+ * decode launch).  d_q, d_out: [total_q][Hq][d]; d_k_new, d_v_new:
+ * [total_q][Hkv][d] bf16 of THIS layer; rows ordered as in the plan.
+ * Capturable in a CUDA graph (the bench does so).  Errors as the calls above. */
+int csv_tail_step(const csv_plan_t* plan, kv_pool_t* pool, int32_t layer, const void* d_q, const void* d_k_new,
+                  const void* d_v_new, const int32_t* d_block_tables, int32_t max_blocks, void* d_out, float* d_lse,
+                  void* stream);
+
 /* ------------------------------------------------------------------------
  * End-to-end convenience with HOST buffers (what bench.py's "e2e" times): one
  * decode tail step of one layer.  Plans from the host lengths, copies

@@ -23,7 +23,7 @@ SYMBOLS = [
     "kv_unpack", "kv_pack_batch", "kv_unpack_batch", "kv_append_tokens", "csv_plan_workspace_bytes",
     "csv_plan_create", "csv_plan_destroy", "csv_plan_info", "csv_plan_total_q", "csv_plan_decode_items",
     "csv_plan_append_items", "paged_decode_attn", "paged_decode_step", "append_prefill_attn", "csv_tail_step_host_workspace_bytes",
-    "csv_tail_step_host", "kv_handoff_direct", "kv_handoff_direct_batch", "csv_ipc_export", "csv_ipc_open", "csv_ipc_close",
+    "csv_tail_step_host", "kv_handoff_direct", "kv_handoff_direct_batch", "csv_ipc_export", "csv_ipc_open", "csv_ipc_close", "csv_tail_step",
 ]
 IPC_HANDLE_BYTES = 64
 
@@ -95,6 +95,7 @@ def lib():
             "paged_decode_attn": (ctypes.c_int, [vp, vp, i32, vp, vp, i32, vp, vp, vp]),
             "append_prefill_attn": (ctypes.c_int, [vp, vp, i32, vp, vp, i32, vp, vp, vp]),
             "paged_decode_step": (ctypes.c_int, [vp, vp, i32, vp, vp, vp, vp, i32, vp, vp, vp]),
+            "csv_tail_step": (ctypes.c_int, [vp, vp, i32, vp, vp, vp, vp, i32, vp, vp, vp]),
             "csv_tail_step_host_workspace_bytes": (sz, [pshape, pi32, i32, i32, i32]),
             "csv_tail_step_host": (ctypes.c_int, [vp, i32, pshape, i32, pi32, vp, vp, vp, pi32, i32, i32, vp, sz, vp,
                                                   vp, vp]),
@@ -371,6 +372,11 @@ def paged_decode_step(plan, pool, layer, d_q, d_k_new, d_v_new, d_block_tables, 
     _check("paged_decode_step", lib().paged_decode_step(plan.handle, pool.handle, layer, _ptr(d_q), _ptr(d_k_new),
                                                         _ptr(d_v_new), _ptr(d_block_tables), max_blocks, _ptr(d_out),
                                                         _ptr(d_lse), _stream(stream)))
+
+
+def csv_tail_step(plan, pool, layer, d_q, d_k_new, d_v_new, d_block_tables, max_blocks, d_out, d_lse, stream=None):
+    _check("csv_tail_step", lib().csv_tail_step(plan.handle, pool.handle, layer, _ptr(d_q), _ptr(d_k_new), _ptr(d_v_new),
+                                                _ptr(d_block_tables), max_blocks, _ptr(d_out), _ptr(d_lse), _stream(stream)))
 
 
 def append_prefill_attn(plan, pool, layer, d_q, d_block_tables, max_blocks, d_out, d_lse, stream=None):

@@ -251,6 +251,33 @@ int kv_append_tokens(kv_pool_t* dst, const csv_plan_t* plan, const void* d_k_new
     return launch_append_tokens(dst, plan, d_k_new, d_v_new, d_block_tables, max_blocks, stream);
 }
 
+// The layer `layer` of a pool as a 1-layer pool (descriptor + base only; the allocator state is neither copied nor used).
+static kv_pool layer_view_of(const kv_pool* pool, int layer) {
+    kv_pool v;
+    v.desc = pool->desc;
+    v.desc.num_layers = 1;
+    v.bytes = 0;
+    v.used = 0;
+    v.d_base = pool->d_base + (size_t)layer * pool->desc.num_blocks * 2 * pool->desc.num_kv_heads *
+                                  csv_tile_bytes(pool->desc.head_dim);
+    return v;
+}
+
+int csv_tail_step(const csv_plan_t* plan, kv_pool_t* pool, int32_t layer, const void* d_q, const void* d_k_new,
+                  const void* d_v_new, const int32_t* d_block_tables, int32_t max_blocks, void* d_out, float* d_lse,
+                  void* stream) {
+    const int rc = check_attn_args(plan, pool, layer, d_q, d_block_tables, max_blocks, d_out, d_lse);
+    if (rc != CSV_OK) return rc;
+    if (!d_k_new || !d_v_new || !aligned(d_k_new, 16) || !aligned(d_v_new, 16)) return CSV_E_INVAL;
+    if (plan->append_items.empty())   // decode rows only: the KV write rides in the decode launch
+        return launch_decode(plan, pool, layer, d_q, d_block_tables, max_blocks, d_out, d_lse, stream, d_k_new, d_v_new);
+    kv_pool view = layer_view_of(pool, layer);
+    int r = launch_append_tokens(&view, plan, d_k_new, d_v_new, d_block_tables, max_blocks, stream);
+    if (r == CSV_OK) r = launch_decode(plan, &view, 0, d_q, d_block_tables, max_blocks, d_out, d_lse, stream);
+    if (r == CSV_OK) r = launch_append_attn(plan, &view, 0, d_q, d_block_tables, max_blocks, d_out, d_lse, stream);
+    return r;
+}
+
 // ---- host-buffer tail step (bench.py "e2e") ---------------------------------------------------
 struct TailLayout {
     size_t plan, q, k, v, tables, out, lse, total;
@@ -290,7 +317,8 @@ int csv_tail_step_host(kv_pool_t* pool, int32_t layer, const csv_attn_shape* sha
     if (!pool || !shape || batch <= 0 || !h_kv_lens || !h_q || !h_k_new || !h_v_new || !h_block_tables || !h_out ||
         !h_lse || !d_workspace || !aligned(d_workspace, 128) || max_blocks <= 0)
         return CSV_E_INVAL;
-    if (layer < 0 || layer >= pool->desc.num_layers) return CSV_E_INVAL;
+    if (layer < 0 || layer >= pool->desc.num_layers || !same_shape(pool->desc, *shape)) return CSV_E_INVAL;
+    if (shape->num_q_heads <= 0 || shape->num_q_heads % shape->num_kv_heads != 0) return CSV_E_INVAL;
     // The plan's size is not known before it is built, so the fixed-size buffers sit in front of it: their copies
     // are enqueued first and fly while the host plans.
     const size_t qb = (size_t)batch * shape->num_q_heads * shape->head_dim * 2;
@@ -316,10 +344,7 @@ int csv_tail_step_host(kv_pool_t* pool, int32_t layer, const csv_attn_shape* sha
         return rc;
     }
     // the new token's K/V go to `layer` of the pool: view that layer as a 1-layer pool
-    kv_pool layer_view = *pool;
-    layer_view.desc.num_layers = 1;
-    layer_view.d_base = pool->d_base + (size_t)layer * pool->desc.num_blocks * 2 * pool->desc.num_kv_heads *
-                                           csv_tile_bytes(pool->desc.head_dim);
+    kv_pool layer_view = layer_view_of(pool, layer);
     if (rc == CSV_OK)   // new-token KV write fused into the decode launch
         rc = paged_decode_step(plan, &layer_view, 0, ws + L.q, ws + L.k, ws + L.v, (const int32_t*)(ws + L.tables), max_blocks,
                                ws + L.out, (float*)(ws + L.lse), stream);

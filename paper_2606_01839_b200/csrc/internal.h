@@ -123,7 +123,7 @@ int launch_append_attn(const csv_plan* plan, const kv_pool* pool, int layer, con
                        int max_blocks, void* out, float* lse, void* stream);
 int launch_append_attn_tc2(const csv_plan* plan, const kv_pool* pool, int layer, const void* q, const int32_t* tables,
                            int max_blocks, void* out, float* lse, void* stream);
-int csv_query_num_sms();
+int csv_query_num_sms();   // SM count of the current device, 148 if none is usable
 csv_plan* csv_plan_build_host(const csv_attn_shape* shape, const int32_t* h_q_lens, const int32_t* h_kv_lens,
                               int32_t batch, int32_t max_partition_tokens, int* err);
-bool csv_shape_ok(const kv_pool_desc* s, bool need_blocks);   // SM count of the current device, 148 if none is usable
+bool csv_shape_ok(const kv_pool_desc* s, bool need_blocks);   // supported (Hkv, d, bs, dtype); need_blocks: num_blocks > 0 too

@@ -55,7 +55,14 @@ static void plan_decode(csv_plan* p) {
 
     int64_t base = 0;   // first unit of the current (conv, head) segment
     int64_t w = 0;      // worker whose share contains `pos`
-    auto share_start = [&](int64_t k) { return (k * units) / W; };
+    // share k starts at floor(k * units / W) = k * sq + floor(k * sr / W): stepped without a division per item
+    // (this loop is on the host path of every tail step)
+    const int64_t sq = units / W, sr = units % W;
+    int64_t next_start = sq, next_rem = sr;   // start of share w + 1, and (w + 1) * sr mod W
+    if (next_rem >= W) {
+        next_rem -= W;
+        ++next_start;
+    }
     for (int b = 0; b < p->batch; ++b) {
         if (p->q_lens[b] != 1) continue;
         const int nblk = (p->kv_lens[b] + CSV_BLOCK_SIZE - 1) / CSV_BLOCK_SIZE;
@@ -64,11 +71,17 @@ static void plan_decode(csv_plan* p) {
             int blk = 0;
             while (blk < nblk) {
                 const int64_t pos = base + blk;
-                while (w + 1 < W && share_start(w + 1) <= pos) {   // advance to the worker owning pos
+                while (w + 1 < W && next_start <= pos) {   // advance to the worker owning pos
                     ++w;
                     p->worker_begin[(size_t)w] = (int32_t)p->decode_items.size();
+                    next_start += sq;
+                    next_rem += sr;
+                    if (next_rem >= W) {
+                        next_rem -= W;
+                        ++next_start;
+                    }
                 }
-                const int64_t share_end = share_start(w + 1);   // == units for the last worker
+                const int64_t share_end = w + 1 < W ? next_start : units;   // start of share w + 1
                 int end = (int)std::min<int64_t>(nblk, share_end - base);
                 end = std::min(end, blk + part_blocks);
                 DecodeItem it{};

@@ -98,6 +98,12 @@ class TailWorkload:
         B.paged_decode_step(self.plan, self.pool, layer, self.d_q, self.d_k_new[layer * per_layer:],
                             self.d_v_new[layer * per_layer:], self.d_tables, self.max_blocks, self.d_out, self.d_lse, stream)
 
+    def tail_step(self, layer=0, stream=None):
+        """One mixed tail step in one call: every new row's K/V write, decode attention, append attention."""
+        per_layer = self.total_q * self.Hkv * self.d
+        B.csv_tail_step(self.plan, self.pool, layer, self.d_q, self.d_k_new[layer * per_layer:],
+                        self.d_v_new[layer * per_layer:], self.d_tables, self.max_blocks, self.d_out, self.d_lse, stream)
+
     def append(self, layer=0, stream=None):
         B.append_prefill_attn(self.plan, self.pool, layer, self.d_q, self.d_tables, self.max_blocks, self.d_out,
                               self.d_lse, stream)

@@ -131,3 +131,51 @@ def test_fused_decode_step_writes_the_token_and_attends_to_it(oracle, Hq, Hkv, d
     assert np.array_equal(dev_to_u16(sc.d_image), full), "pool after the fused step differs from the oracle's scatter"
     O_ref, LSE_ref = oracle_attention(sc, [1] * n, q)
     assert_close(bf16_dev_to_f64(d_out), d_lse.cpu().numpy().astype(np.float64), O_ref, LSE_ref, what="fused step")
+
+
+def test_tail_step_mixed_batch_one_call(oracle):
+    """csv_tail_step (PAPER.md:112 collocated iteration): decode rows and appended chunks of one step in
+    one call on layer 1 of a 2-layer pool: every new row's K/V lands where the oracle's scatter puts it (whole pool
+    image, layer 0 untouched), O / LSE match the oracle on the full cache; a pure-decode plan takes the fused path."""
+    from harness import dev_to_u16
+    rng = np.random.default_rng(91)
+    Hq, Hkv, d, NL, layer = 32, 8, 128, 2, 1
+    kv_lens = [700, 33, 2049, 300, 16, 1, 4097, 129]
+    q_lens = [1, 32, 1, 257, 1, 1, 40, 0]
+    sc = Scenario(oracle, rng, Hq, Hkv, d, kv_lens, NL=NL, poison=True)
+    full = sc.image.copy()
+    for b, (t, m) in enumerate(zip(kv_lens, q_lens)):
+        full = oracle.scatter(full, NL, sc.num_blocks, Hkv, d, sc.K[b], sc.V[b], t, 0, sc.tables[b])
+        # the cache before the step: layer 0 complete, layer 1 without the step's own rows
+        K0, V0 = sc.K[b].copy(), sc.V[b].copy()
+        sc.image = oracle.scatter(sc.image, NL, sc.num_blocks, Hkv, d, K0[:, :t - m], V0[:, :t - m], t - m, 0, sc.tables[b]) \
+            if t - m > 0 else sc.image
+        if m > 0:   # layer 0 already holds the step's rows (an earlier layer of the same step), layer 1 does not
+            own = oracle.scatter(np.full_like(sc.image, 0), NL, sc.num_blocks, Hkv, d, K0[:, t - m:], V0[:, t - m:], m, t - m,
+                                 sc.tables[b])
+            mask = oracle.scatter(np.full_like(sc.image, 0), NL, sc.num_blocks, Hkv, d, np.full_like(K0[:, t - m:], 1),
+                                  np.full_like(V0[:, t - m:], 1), m, t - m, sc.tables[b]).astype(bool)
+            half = sc.image.size // NL
+            mask[half:] = False                      # only layer 0
+            sc.image = np.where(mask, own, sc.image)
+    sc.upload()
+    k_new = np.concatenate([sc.K[b][layer, t - m:t] for b, (t, m) in enumerate(zip(kv_lens, q_lens)) if m > 0])
+    v_new = np.concatenate([sc.V[b][layer, t - m:t] for b, (t, m) in enumerate(zip(kv_lens, q_lens)) if m > 0])
+    total_q = sum(q_lens)
+    q = synth.normal_bf16(rng, (total_q, Hq, d))
+    shape = B.attn_shape(Hq, Hkv, d)
+    ws = torch.empty(B.csv_plan_workspace_bytes(shape, q_lens, kv_lens), dtype=torch.uint8, device="cuda")
+    plan = B.Plan(shape, q_lens, kv_lens, 0, ws)
+    d_out = torch.full((total_q, Hq, d), 0x7FC0, dtype=torch.int16, device="cuda")
+    d_lse = torch.full((total_q, Hq), float("nan"), dtype=torch.float32, device="cuda")
+    B.csv_tail_step(plan, sc.pool, layer, u16_dev(q), u16_dev(k_new), u16_dev(v_new), sc.d_tables, sc.max_blocks, d_out, d_lse)
+    torch.cuda.synchronize()
+    got = dev_to_u16(sc.d_image)
+    assert np.array_equal(got, full), "pool after csv_tail_step differs from the oracle's scatter (%d elements)" % int(
+        (got != full).sum())
+    O_ref, LSE_ref = oracle_attention(sc, q_lens, q, layer=layer)
+    assert_close(bf16_dev_to_f64(d_out), d_lse.cpu().numpy().astype(np.float64), O_ref, LSE_ref, what="csv_tail_step")
+    with pytest.raises(B.CsvError):
+        B.csv_tail_step(plan, sc.pool, 2, u16_dev(q), u16_dev(k_new), u16_dev(v_new), sc.d_tables, sc.max_blocks, d_out, d_lse)
+    with pytest.raises(B.CsvError):
+        B.csv_tail_step(plan, sc.pool, layer, u16_dev(q), None, u16_dev(v_new), sc.d_tables, sc.max_blocks, d_out, d_lse)
