@@ -179,3 +179,66 @@ def test_tail_step_mixed_batch_one_call(oracle):
         B.csv_tail_step(plan, sc.pool, 2, u16_dev(q), u16_dev(k_new), u16_dev(v_new), sc.d_tables, sc.max_blocks, d_out, d_lse)
     with pytest.raises(B.CsvError):
         B.csv_tail_step(plan, sc.pool, layer, u16_dev(q), None, u16_dev(v_new), sc.d_tables, sc.max_blocks, d_out, d_lse)
+
+
+def test_append_spike_sweep_sees_every_block(oracle):
+    """SURVEY §8c item 1 for the tcgen05 kernel: one key carries ~all the weight for every row that may see it and its V
+    is a +-1 pattern; the spike sits on the first / last block of each KV partition, around the prefix / chunk boundary
+    and on the diagonal.  A dropped, duplicated or misplaced 16-token block (or a wrong mask edge) is an O(1) error."""
+    rng = np.random.default_rng(137)
+    Hq, Hkv, d, L, m, G = 32, 8, 128, 6001, 40, 4          # 160 stacked rows per KV head: tile A full, tile B ragged
+    P = L - m
+    positions = sorted(set([0, 15, 16, 2047, 2048, 2049, 4095, 4096, P - 16, P - 1, P, P + 1, P + 17, L - 2, L - 1,
+                            (L // 16) * 16, (L // 16) * 16 - 1] + list(rng.integers(0, L, size=5))))
+    n = len(positions)
+    sc = Scenario(oracle, rng, Hq, Hkv, d, [L] * n)
+    # all rows of a chunk share a direction per KV group (plus noise), so one key can dominate every row of the group
+    base = rng.standard_normal((n, Hkv, d)).astype(np.float32)
+    qf = np.repeat(base, G, axis=1)[:, None] + 0.3 * rng.standard_normal((n, m, Hq, d)).astype(np.float32)
+    q = synth.f32_to_bf16_bits(qf.reshape(n * m, Hq, d))
+    pattern = np.where(rng.random((n, Hkv, d)) < 0.5, -1.0, 1.0).astype(np.float32)
+    for b, j in enumerate(positions):
+        for g in range(Hkv):
+            u = base[b, g]
+            sc.K[b][0, j, g] = synth.f32_to_bf16_bits(u * (22.0 * np.sqrt(d) / np.dot(u, u)))
+            sc.V[b][0, j, g] = synth.f32_to_bf16_bits(pattern[b, g])
+    sc.commit().upload()
+    O, LSE, info = run_attention(sc, [m] * n, q, mpt=2048, which="append")
+    assert info["n_append_chunks"] == n
+    O_ref, LSE_ref = oracle_attention(sc, [m] * n, q)
+    assert_close(O, LSE, O_ref, LSE_ref, what="append spike sweep")
+    hit = 0
+    for b, j in enumerate(positions):
+        for i in range(m):
+            if j > P + i:
+                continue                                     # the spike is behind the diagonal for this row
+            for h in range(Hq):
+                r = b * m + i
+                if np.abs(O_ref[r, h] - pattern[b, h // G]).max() < 1e-3:
+                    assert np.abs(O[r, h] - pattern[b, h // G]).max() <= 1e-2
+                    hit += 1
+    assert hit > 0.5 * n * m * Hq * 0.8                      # most visible (row, head) pairs are dominated by the spike
+
+
+def test_append_is_bit_identical_under_block_permutation_and_reruns(oracle):
+    # S8 for the append path: the schedule depends only on the lengths -> same bits wherever the blocks sit, run to run
+    convs = [(3000, 100), (17, 33), (5000, 40), (0, 64)]
+    q_lens = [m for _, m in convs]
+    kv = [P + m for P, m in convs]
+    outs = []
+    for perm_seed in (1, 2):
+        rng = np.random.default_rng(140)
+        sc = Scenario(oracle, rng, 32, 8, 128, kv)
+        q = synth.normal_bf16(rng, (sum(q_lens), 32, 128))
+        order = synth.shuffled_free_order(np.random.default_rng(perm_seed), sc.num_blocks)
+        pos = 0
+        for i, t in enumerate(kv):
+            nb = synth.blocks_for(t)
+            sc.tables[i] = order[pos:pos + nb].copy()
+            pos += nb
+        sc.commit().upload()
+        for _ in range(2):
+            O, LSE, _ = run_attention(sc, q_lens, q, mpt=1024, which="append")
+            outs.append((O.copy(), LSE.copy()))
+    for O, LSE in outs[1:]:
+        assert np.array_equal(O, outs[0][0]) and np.array_equal(LSE, outs[0][1])
