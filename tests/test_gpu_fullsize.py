@@ -159,3 +159,82 @@ def test_turn1_prefill_chunk_8192_through_append_prefill_attn(oracle):
         O, LSE = bf16_dev_to_f64(app.d_out), app.d_lse.cpu().numpy().astype(np.float64)
         assert np.all(np.isfinite(O)) and np.all(np.isfinite(LSE))
         check_rows(oracle, app, 0, [(0, 0), (0, 1), (0, 127), (0, 4096), (0, 8191)], O, LSE, "prefill chunk P=%d" % P)
+
+
+def test_spike_sweep_at_131072_tokens_decode_and_append(oracle):
+    """SURVEY §8c item 1 at config 5's length: with N(0,1) data a dropped 16-token block is invisible to the 1e-2 gate once
+    L >~ 8k, so one key per (conversation, KV head) is made to carry ~all the weight (score ~30 against a log-sum-exp of
+    ~12.3 for the other 131071 keys) with a +-1 pattern as its V: closed-form answer, no fp64 run.  The spikes sit on the
+    first and last block of split-K partitions taken from the plan, at both ends of the sequence and at random places.
+    They are written into the device pool at the oracle's addresses (O2's formula), not through the library."""
+    cfg = synth.CONFIGS[5]
+    Hq, Hkv, d, G, L, n = cfg["Hq"], cfg["Hkv"], cfg["d"], cfg["Hq"] // cfg["Hkv"], 131072, 6
+    m = 24                                                   # appended rows of the second plan (conversations 0, 1)
+    wl = workloads.TailWorkload(Hq, Hkv, d, [1] * n, [L] * n, seed=77, slack=0.02)
+    items, _ = wl.plan.decode_items()
+    rng = np.random.default_rng(78)
+    q = synth.bf16_bits_to_f32(dev_to_u16(wl.d_q).reshape(n, Hq, d))
+    app = wl.with_q_lens([m, m] + [0] * (n - 2))
+    qa_bits = dev_to_u16(app.d_q).reshape(2 * m, Hq, d).copy()
+    pos = np.zeros((n, Hkv), dtype=np.int64)
+    pattern = np.where(rng.random((n, Hkv, d)) < 0.5, -1.0, 1.0).astype(np.float32)
+    pool16 = wl.d_pool.view(torch.int16)
+    spike_k = np.zeros((n, Hkv, d), dtype=np.float32)
+    for b in range(n):
+        for g in range(Hkv):
+            mine = items[(items[:, 0] == b) & (items[:, 1] == g)]
+            assert len(mine) >= 8                             # split-K really cuts this sequence
+            part = mine[int(rng.integers(0, len(mine)))]
+            choice = int(rng.integers(0, 6))
+            j = [int(part[2]) * 16, int(part[3]) * 16 - 1, 0, L - 1, int(rng.integers(0, L)), int(part[2]) * 16 + 15][choice]
+            if b < 2:
+                j = min(j, L - m - 1)                         # visible to every appended row of conversations 0, 1
+            pos[b, g] = j
+            dirv = q[b, g * G:(g + 1) * G].sum(axis=0)
+            if b < 2:                                         # the appended rows share this direction (see below)
+                dirv = dirv / np.linalg.norm(dirv) * np.sqrt(d)
+            spike_k[b, g] = dirv * (30.0 * np.sqrt(d) / np.dot(dirv, dirv) * (G if b >= 2 else 1.0))
+            kb, vb = synth.f32_to_bf16_bits(spike_k[b, g]), synth.f32_to_bf16_bits(pattern[b, g])
+            blk, slot = int(wl.tables[b][j // 16]), j % 16
+            ka = np.array([oracle.pool_addr(wl.num_blocks, Hkv, d, 0, blk, 0, g, slot, c) for c in range(d)], dtype=np.int64)
+            va = np.array([oracle.pool_addr(wl.num_blocks, Hkv, d, 0, blk, 1, g, slot, c) for c in range(d)], dtype=np.int64)
+            pool16[torch.from_numpy(ka).cuda()] = torch.from_numpy(kb.view(np.int16)).cuda()
+            pool16[torch.from_numpy(va).cuda()] = torch.from_numpy(vb.view(np.int16)).cuda()
+    spike_k = synth.bf16_bits_to_f32(synth.f32_to_bf16_bits(spike_k))
+    # ---- decode: 6 x 131072 ----
+    wl.d_out.fill_(0x7FC0)
+    wl.decode()
+    torch.cuda.synchronize()
+    O, LSE = bf16_dev_to_f64(wl.d_out), wl.d_lse.cpu().numpy().astype(np.float64)
+    checked = 0
+    for b in range(n):
+        for h in range(Hq):
+            s = float(np.dot(q[b, h].astype(np.float64), spike_k[b, h // G].astype(np.float64)) / np.sqrt(d))
+            if s >= 22.0:                                     # others weigh <= exp(13.5 - 22) = 2e-4
+                assert np.abs(O[b, h] - pattern[b, h // G]).max() <= 1e-2, (b, h, int(pos[b, h // G]), s)
+                assert s - 1e-3 <= LSE[b, h] <= s + 1e-3 + np.exp(13.5 - s), (b, h, s, LSE[b, h])
+                checked += 1
+    assert checked >= 0.5 * n * Hq
+    # ---- append on the same pool: rows of conversations 0 and 1 all point along the group's direction ----
+    qa = np.zeros((2 * m, Hq, d), dtype=np.float32)
+    for b in range(2):
+        for h in range(Hq):
+            u = spike_k[b, h // G] / np.linalg.norm(spike_k[b, h // G]) * np.sqrt(d)
+            qa[b * m:(b + 1) * m, h] = u + 0.3 * rng.standard_normal((m, d)).astype(np.float32)
+    qa_bits = synth.f32_to_bf16_bits(qa)
+    app.d_q.copy_(torch.from_numpy(qa_bits.view(np.int16)).cuda().view_as(app.d_q))
+    app.d_out.fill_(0x7FC0)
+    app.append()
+    torch.cuda.synchronize()
+    O, LSE = bf16_dev_to_f64(app.d_out), app.d_lse.cpu().numpy().astype(np.float64)
+    qa = synth.bf16_bits_to_f32(qa_bits)
+    checked = 0
+    for r in range(2 * m):
+        b = r // m
+        for h in range(Hq):
+            s = float(np.dot(qa[r, h].astype(np.float64), spike_k[b, h // G].astype(np.float64)) / np.sqrt(d))
+            if s >= 22.0:
+                assert np.abs(O[r, h] - pattern[b, h // G]).max() <= 1e-2, (r, h, int(pos[b, h // G]), s)
+                assert s - 1e-3 <= LSE[r, h] <= s + 1e-3 + np.exp(13.5 - s)
+                checked += 1
+    assert checked >= 0.9 * 2 * m * Hq
