@@ -239,7 +239,8 @@ def tail_extra(k, iters=10):
     import torch
     from paper_2606_01839_b200 import workloads
 
-    wl = workloads.config_tail_workload(k)
+    full5 = k == 5 and torch.cuda.mem_get_info()[0] > 85e9      # all 8 layers of config 5 (~69 GB of KV) when they fit
+    wl = workloads.config_tail_workload(k, layers=8) if full5 else workloads.config_tail_workload(k)
     out = {"workload": "configs[%d] %s" % (k - 1, __import__("paper_2606_01839_b200.synth", fromlist=["x"]).CONFIGS[k]["name"])}
     app = wl if k == 3 else wl.with_q_lens(workloads.config5_append_q_lens())
     if k == 5:
@@ -265,6 +266,25 @@ def tail_extra(k, iters=10):
 
     both_ms, _ = time_calls(both, max(3, iters // 2))
     out.update(decode_plus_append_overlapped_ms=both_ms)
+    if full5:
+        # configs[4]'s whole step: decode for all 16 conversations + the 4 appended chunks, on each of the 8 layers
+        def step8():
+            for layer in range(8):
+                wl.decode(layer=layer)
+                app.append(layer=layer)
+        g8 = torch.cuda.CUDAGraph()
+        step8()
+        torch.cuda.synchronize()
+        with torch.cuda.graph(g8):
+            step8()
+        s8_ms, _ = time_calls(g8.replay, 3, 1)
+
+        def dec8():
+            for layer in range(8):
+                wl.decode(layer=layer)
+        d8_ms, _ = time_calls(dec8, 3, 1)
+        out.update(layers_in_pool=8, pool_gb=wl.pool_bytes / 1e9, step_8_layers_ms=s8_ms, decode_8_layers_ms=d8_ms,
+                   decode_8_layers_gbs=8 * wl.decode_kv_bytes() / d8_ms / 1e6)
     if k == 3:
         # the whole mixed step in one call (csv_tail_step: KV write of all 9347 new rows + decode + append), replayed
         # from a CUDA graph as a serving loop would
