@@ -227,7 +227,9 @@ int kv_handoff_direct_batch(kv_pool_t* dst, int32_t n, const void* const* h_d_k,
  *   any channel (torch.distributed object collectives in the tests).
  * csv_ipc_open: in another process, maps the allocation (peer access enabled
  *   lazily when it lives on another GPU) and returns base + offset.
- * csv_ipc_close: unmaps; d_ptr is what csv_ipc_open returned.
+ *   Opens of the same allocation are counted (several exported pointers may
+ *   share one allocation); the mapping goes away with the last close.
+ * csv_ipc_close: d_ptr is what csv_ipc_open returned (one close per open).
  * Errors: CSV_E_INVAL bad argument / unknown pointer, CSV_E_CUDA otherwise. */
 #define CSV_IPC_HANDLE_BYTES 64
 int csv_ipc_export(const void* d_ptr, void* out_handle, uint64_t* out_offset);

@@ -124,11 +124,14 @@ static cu_get_range_fn driver_get_range() {
     return fn;
 }
 
-struct ipc_mapping {
-    void* user;   // what csv_ipc_open returned
-    void* base;   // what cudaIpcOpenMemHandle returned
+// One entry per allocation opened in this process.  The driver refuses to map the same handle twice, and several
+// exported pointers often share one cudaMalloc allocation (the caller's caching allocator), so opens are counted.
+struct ipc_region {
+    uint8_t handle[CSV_IPC_HANDLE_BYTES];
+    void* base;                 // what cudaIpcOpenMemHandle returned
+    std::vector<void*> users;   // pointers csv_ipc_open handed out (base + offset), one per open
 };
-static std::vector<ipc_mapping> g_ipc;   // host calls are thread-compatible, not thread-safe (header)
+static std::vector<ipc_region> g_ipc;   // host calls are thread-compatible, not thread-safe (header)
 
 int csv_ipc_export(const void* d_ptr, void* out_handle, uint64_t* out_offset) {
     if (!d_ptr || !out_handle || !out_offset) return CSV_E_INVAL;
@@ -147,24 +150,37 @@ int csv_ipc_export(const void* d_ptr, void* out_handle, uint64_t* out_offset) {
 
 int csv_ipc_open(const void* handle, uint64_t offset, void** out_d_ptr) {
     if (!handle || !out_d_ptr) return CSV_E_INVAL;
+    for (ipc_region& r : g_ipc) {
+        if (memcmp(r.handle, handle, CSV_IPC_HANDLE_BYTES) == 0) {
+            r.users.push_back((uint8_t*)r.base + offset);
+            *out_d_ptr = r.users.back();
+            return CSV_OK;
+        }
+    }
     cudaIpcMemHandle_t h;
     memcpy(&h, handle, sizeof(h));
     void* base = nullptr;
     CSV_CUDA_TRY(cudaIpcOpenMemHandle(&base, h, cudaIpcMemLazyEnablePeerAccess));
-    ipc_mapping m;
-    m.base = base;
-    m.user = (uint8_t*)base + offset;
-    g_ipc.push_back(m);
-    *out_d_ptr = m.user;
+    ipc_region r;
+    memcpy(r.handle, handle, CSV_IPC_HANDLE_BYTES);
+    r.base = base;
+    r.users.push_back((uint8_t*)base + offset);
+    *out_d_ptr = r.users.back();
+    g_ipc.push_back(r);
     return CSV_OK;
 }
 
 int csv_ipc_close(void* d_ptr) {
     for (size_t i = 0; i < g_ipc.size(); ++i) {
-        if (g_ipc[i].user == d_ptr) {
-            void* base = g_ipc[i].base;
-            g_ipc.erase(g_ipc.begin() + (long)i);
-            CSV_CUDA_TRY(cudaIpcCloseMemHandle(base));
+        std::vector<void*>& u = g_ipc[i].users;
+        for (size_t k = 0; k < u.size(); ++k) {
+            if (u[k] != d_ptr) continue;
+            u.erase(u.begin() + (long)k);
+            if (u.empty()) {
+                void* base = g_ipc[i].base;
+                g_ipc.erase(g_ipc.begin() + (long)i);
+                CSV_CUDA_TRY(cudaIpcCloseMemHandle(base));
+            }
             return CSV_OK;
         }
     }

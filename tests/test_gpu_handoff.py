@@ -2,6 +2,8 @@
 oracle's reference scatter (O3) and staging formula.  Bit-exact, whole pool image compared
 (a stray write anywhere is a mismatch).  PAPER.md:150 §4 "transferred once to the bound decoder".
 """
+import os
+
 import numpy as np
 import pytest
 import torch
@@ -244,3 +246,26 @@ def test_direct_handoff_into_another_process_pool_over_cuda_ipc(oracle):
     expected = oracle.scatter(image, NL, nb, Hkv, d, K, V, tokens, off, ids)
     assert np.array_equal(dev_to_u16(d_image), expected)
     assert bool((slab[:4096] == 0x2222).all()) and bool((slab[4096 + n:] == 0x2222).all())
+
+
+def test_handoff_across_two_ranks_direct_and_staged():
+    """paper_2606_01839_b200.handoff_p2p under torchrun with two ranks (prefiller, decoder): on this one-GPU box both share
+    the device; with two GPUs the same program pushes over NVLink.  It exits non-zero unless both routes leave the
+    decoder's pool bit-identical to a local handoff of the same K/V."""
+    import json
+    import socket
+    import subprocess
+    import sys
+
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), "-m", "paper_2606_01839_b200.handoff_p2p", "--tokens", "1000", "--layers", "4",
+           "--convs", "5", "--iters", "1"]
+    r = subprocess.run(cmd, cwd=root, capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-2000:]
+    line = [ln for ln in r.stdout.splitlines() if ln.startswith("{")][-1]
+    out = json.loads(line)
+    assert out["bit_exact_direct"] and out["bit_exact_staged"] and out["convs"] == 5
