@@ -38,6 +38,7 @@ struct AppendTc2Params {
     float* pml;
     int32_t max_blocks, Hq, Hkv, G;
     float scale_log2;
+    uint32_t* sched;   // [0] next item of the work queue (beyond the first gridDim.x), [1] CTAs that have finished
 };
 
 constexpr uint32_t kOffQ2 = 0;                           // 2 tiles x [2 halves][128 rows][128 B]
@@ -83,7 +84,13 @@ __global__ void __launch_bounds__(kT2Threads, 1) append_tc2_kernel(const __grid_
     uint32_t kc = 0;             // K/V chunks pushed through the rings so far (all roles agree)
     uint32_t tcnA = 0, tcnB = 0;   // chunks each tile has processed so far (tile B skips items without rows for it)
 
-    for (int it = blockIdx.x; it < p.n_items; it += gridDim.x) {
+    // Work queue: CTA c starts with item c and then takes the next unclaimed one (items are sorted longest first, so
+    // this is LPT scheduling).  Thread 0 claims the NEXT item while the current one runs; the index travels through
+    // shared memory under the barrier that ends the Q staging.
+    uint32_t* next_slot = tmem_slot + 2;   // [2] in the barrier block
+    int it = blockIdx.x, par = 0;
+    while (it < p.n_items) {
+        if (threadIdx.x == 0) next_slot[par] = gridDim.x + atomicAdd(p.sched, 1u);
         const int4 i0 = __ldg(reinterpret_cast<const int4*>(p.items + it));
         const int4 i1 = __ldg(reinterpret_cast<const int4*>(p.items + it) + 1);
         const int4 i2 = __ldg(reinterpret_cast<const int4*>(p.items + it) + 2);
@@ -116,6 +123,7 @@ __global__ void __launch_bounds__(kT2Threads, 1) append_tc2_kernel(const __grid_
         tc_fence_before();
         __syncthreads();   // Q staged; the previous item's epilogues have finished reading O
         tc_fence_after();
+        const int it_next = (int)next_slot[par];
 
         if (warp == 8) {
             // ================= producer =================
@@ -365,6 +373,12 @@ __global__ void __launch_bounds__(kT2Threads, 1) append_tc2_kernel(const __grid_
         tcnA += nch;
         if (hasB) tcnB += nch;
         tc_fence_before();   // order this item's TMEM traffic before the next item's barrier
+        it = it_next;
+        par ^= 1;
+    }
+    if (threadIdx.x == 0 && atomicAdd(p.sched + 1, 1u) == gridDim.x - 1) {   // last CTA out: queue back to zero
+        atomicExch(p.sched, 0u);
+        atomicExch(p.sched + 1, 0u);
     }
     __syncthreads();
     if (warp == 9) tmem_dealloc(tmem, kTmemCols2);
@@ -390,6 +404,7 @@ int launch_append_attn_tc2(const csv_plan* plan, const kv_pool* pool, int layer,
     p.Hkv = plan->shape.num_kv_heads;
     p.G = p.Hq / p.Hkv;
     p.scale_log2 = (float)(1.4426950408889634 / sqrt((double)s.head_dim));
+    p.sched = reinterpret_cast<uint32_t*>(plan->d_ws + plan->lay.append_sched);
     static bool attr_set = false;
     if (!attr_set) {
         CSV_CUDA_TRY(cudaFuncSetAttribute(append_tc2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes2));

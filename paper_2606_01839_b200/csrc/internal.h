@@ -76,6 +76,7 @@ struct PlanLayout {   // byte offsets into the caller's workspace (all 128-byte 
     size_t decode_items, worker_begin, decode_groups, decode_po, decode_pml;
     size_t append_items, append_groups, append_po, append_pml;
     size_t conv_meta;   // int32 [q_start[batch+1] | kv_len[batch] | q_len[batch]]
+    size_t append_sched;   // uint32 [next item, CTAs done]: the append kernel's work queue, zero between launches
     size_t total;
 };
 
