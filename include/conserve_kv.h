@@ -269,10 +269,11 @@ size_t csv_plan_workspace_bytes(const csv_attn_shape* shape, const int32_t* h_q_
  * (128-byte aligned) on `stream`.  q_len[b] must be in [0, kv_len[b]];
  * q_len = 0 rows are inert.  The plan may be used on that stream (or after
  * synchronising with it) until destroyed; the workspace must outlive it.
- * Calls that use one plan share its workspace (split-K partials, the append
- * kernel's work queue): they must be ordered on the device, one after the
- * other (same stream, or events), never concurrent; one plan serves all the
- * layers of a step in turn.
+ * Launches of the SAME call on one plan share workspace (the decode partials;
+ * the append partials and the append kernel's work queue): they must be
+ * ordered on the device (same stream, or events), never concurrent.  A decode
+ * call and an append call of one plan use disjoint regions and may overlap.
+ * One plan serves all the layers of a step in turn.
  * d_workspace = NULL builds a host-only plan (no CUDA call): good for
  * csv_plan_info / csv_plan_*_items, refused (CSV_E_INVAL) by the attention calls.
  * ws_bytes too small -> CSV_E_NOMEM. */
