@@ -173,7 +173,7 @@ __global__ void __launch_bounds__(kT2Threads, 1) append_tc2_kernel(const __grid_
             const uint64_t kd = smem_desc_sw128(sbase + kOffK2, 16, 1024);
             const uint64_t vd = smem_desc_sw128(sbase + kOffV2, 2048, 1024);
             // broadcast through a shuffle: tells the compiler these are warp-uniform, so the per-MMA descriptor words are
-            // formed on the uniform datapath instead of one R2UR chain per MMA (measured: ~114 -> ~50-64 cycles per MMA)
+            // formed on the uniform datapath (UIADD3) instead of one R2UR chain per MMA
             const uint32_t q_lo = __shfl_sync(0xffffffffu, (uint32_t)qd, 0), qk_hi = __shfl_sync(0xffffffffu, (uint32_t)(qd >> 32), 0);
             const uint32_t k_lo = __shfl_sync(0xffffffffu, (uint32_t)kd, 0);
             const uint32_t v_lo = __shfl_sync(0xffffffffu, (uint32_t)vd, 0), v_hi = __shfl_sync(0xffffffffu, (uint32_t)(vd >> 32), 0);
