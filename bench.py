@@ -431,6 +431,13 @@ def run_ours(args):
         return
     peak, peak_src = measured_peaks()
     achieved = kv_bytes / dec_ms / 1e6
+    # host planning (reported apart from kernel time; one plan serves all layers of a step)
+    pt = []
+    for _ in range(21):
+        t0 = time.perf_counter()
+        B.Plan(wl.shape, wl.q_lens, wl.kv_lens).destroy()
+        pt.append((time.perf_counter() - t0) * 1e6)
+    plan_us = sorted(pt)[len(pt) // 2]
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms_step,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
@@ -439,7 +446,8 @@ def run_ours(args):
                    "kv_bytes_per_step_per_gpu": kv_bytes, "kv_tokens": int(sum(wl.kv_lens)), "decode_rows": rows,
                    "l2": "inputs larger than L2 (%.2f GB of KV per step vs 126 MB)" % (kv_bytes / 1e9),
                    "parallelism": "replicas x%d, no collective" % world, "decode_grid": info["decode_grid"],
-                   "decode_items": info["n_decode_items"], "cuda_graph": graph is not None},
+                   "decode_items": info["n_decode_items"], "cuda_graph": graph is not None,
+                   "plan_host_us": plan_us, "plan_host_us_per_layer_of_32": plan_us / 32.0},
         "tokens_per_s": world * rows / ms_step * 1e3, "us_per_step": ms_step * 1e3,
         "pct_of_nominal_8000": 100.0 * value / world / NOMINAL_HBM_GBS,
         "roofline": {"bound": "hbm", "kernel": "decode_kernel<128,3> (+ decode_merge_kernel), per paged_decode_attn call; timed over K back-to-back calls",
