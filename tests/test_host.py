@@ -272,3 +272,30 @@ def test_workspace_bytes_grows_with_partials_and_is_checked():
     assert B.csv_plan_workspace_bytes(sh, [2], [1]) == 0
     kv = [4096] * 4
     assert B.csv_tail_step_host_workspace_bytes(sh, kv, 256) > B.csv_plan_workspace_bytes(sh, [1] * 4, kv)
+
+
+def test_handoff_direct_and_ipc_reject_bad_arguments_before_touching_cuda():
+    pool = mkpool(8, NL=1, Hkv=1, d=64)
+    k = FAKE + (1 << 20)
+    ids = FAKE + (2 << 20)
+    for call in (lambda: B.kv_handoff_direct(pool, k, k, 0, 0, ids, 8, stream=0),          # zero tokens
+                 lambda: B.kv_handoff_direct(pool, k, k, 10, -1, ids, 8, stream=0),
+                 lambda: B.kv_handoff_direct(pool, k + 2, k, 10, 0, ids, 8, stream=0),      # misaligned source
+                 lambda: B.kv_handoff_direct(pool, k, None, 10, 0, ids, 8, stream=0),
+                 lambda: B.kv_handoff_direct(pool, k, k, 10, 0, None, 8, stream=0),
+                 lambda: B.kv_handoff_direct(pool, k, k, 300, 0, ids, 8, stream=0),         # table shorter than ceil(300 / 16)
+                 lambda: B.kv_handoff_direct_batch(pool, [k], [k], [17], [112], [ids], [8], stream=0)):
+        with pytest.raises(B.CsvError) as e:
+            call()
+        assert e.value.code == B.CSV_E_INVAL
+    B.kv_handoff_direct_batch(pool, [k, k], [k, k], [0, 0], [0, 0], [ids, ids], [8, 8], stream=0)   # nothing to do: no launch
+    L = B.lib()
+    off = ctypes.c_uint64()
+    out = ctypes.c_void_p()
+    buf = ctypes.create_string_buffer(B.IPC_HANDLE_BYTES)
+    assert L.csv_ipc_export(None, buf, ctypes.byref(off)) == B.CSV_E_INVAL
+    assert L.csv_ipc_export(ctypes.c_void_p(k), None, ctypes.byref(off)) == B.CSV_E_INVAL
+    assert L.csv_ipc_open(None, 0, ctypes.byref(out)) == B.CSV_E_INVAL
+    assert L.csv_ipc_open(buf, 0, None) == B.CSV_E_INVAL
+    assert L.csv_ipc_close(ctypes.c_void_p(k)) == B.CSV_E_INVAL                   # never opened
+    assert pool.used_blocks == 0
