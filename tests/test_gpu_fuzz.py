@@ -44,3 +44,20 @@ def test_random_tail_step_matches_the_oracle(oracle, seed):
     Hq, Hkv, d, convs, mpt, poison, qscale, v_mean = random_case(seed)
     step_case(oracle, 5000 + seed, Hq, Hkv, d, convs, mpt=mpt, poison=poison, v_mean=v_mean, qscale=qscale,
               what="fuzz %d %s %s mpt=%d poison=%s q x%g" % (seed, (Hq, Hkv, d), convs, mpt, poison, qscale))
+
+
+@pytest.mark.parametrize("seed", range(int(os.environ.get("CSV_FUZZ_CASES", "24")) // 2))
+def test_random_handoff_matches_the_oracle(oracle, seed):
+    """kv_pack -> kv_unpack and kv_handoff_direct, single and batched: random layer counts, head counts, lengths and
+    token offsets (ragged first and last blocks), random 16-bit patterns; whole pool image against the oracle's scatter."""
+    from test_gpu_handoff import handoff_case
+
+    rng = np.random.default_rng(9000 + seed)
+    NL, Hkv, d = int(rng.integers(1, 4)), int(rng.choice([1, 2, 4, 8])), int(rng.choice([64, 128]))
+    n = int(rng.integers(1, 40))
+    convs = []
+    for _ in range(n):
+        tokens = int(rng.choice([1, 2, 15, 16, 17, 31, 32, 33])) if rng.random() < 0.5 else int(rng.integers(1, 200))
+        convs.append((tokens, int(rng.integers(0, 40)) if rng.random() < 0.5 else 0))
+    blocks = sum((o + t + 15) // 16 for t, o in convs) + int(rng.integers(1, 9))
+    handoff_case(oracle, rng, NL, Hkv, d, blocks, convs, batched=bool(rng.random() < 0.6), direct=bool(rng.random() < 0.5))
