@@ -102,6 +102,13 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
+def oracle_logical_kv(oracle, wl, b, layer=0):
+    """cpu_baseline leg only: conversation b's raw pool blocks copied back, gathered (paged -> logical) by the ORACLE."""
+    img = wl.conversation_blocks_host(b, layer)
+    n = len(wl.tables[b])
+    return oracle.gather(img, n, wl.Hkv, wl.d, 0, np.arange(n, dtype=np.int32), wl.kv_lens[b])
+
+
 def oracle_sample(wl, n_conv, layer=0):
     """Time the oracle (fp64, one thread) on the first n_conv conversations of the workload.
     Returns (seconds, KV bytes it read)."""
@@ -111,7 +118,7 @@ def oracle_sample(wl, n_conv, layer=0):
     q_all = wl.d_q.cpu().contiguous().view(-1, wl.Hq, wl.d).numpy().view(np.uint16)
     rows = [b for b in range(len(wl.q_lens)) if wl.q_lens[b] == 1][:n_conv]
     starts = np.concatenate([[0], np.cumsum(wl.q_lens)])
-    data = [(q_all[starts[b]:starts[b] + 1], *wl.logical_kv(oracle, b, layer)) for b in rows]
+    data = [(q_all[starts[b]:starts[b] + 1], *oracle_logical_kv(oracle, wl, b, layer)) for b in rows]
     t0 = time.perf_counter()
     outs = [oracle.attention(q, K, V) for (q, K, V) in data]
     dt = time.perf_counter() - t0

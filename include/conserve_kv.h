@@ -26,6 +26,22 @@
  *    GQA group G = Hq / Hkv in {1, 2, 4, 8}.
  *  - There is no CPU fallback: if no CUDA device / kernel image is usable the
  *    launching calls return CSV_E_CUDA.
+ *  - Devices.  Every call works on the CURRENT device (cudaSetDevice) of the
+ *    calling thread: a pool, a plan and its workspace, and the stream passed
+ *    with them must all belong to the device that is current at the call.  The
+ *    usual deployment is one process per GPU (§5.1 "each served
+ *    model replica occupies one GPU").  A process that drives several GPUs may
+ *    do so, one device current at a time: the library keeps its per-device
+ *    state (kernel attributes, SM count, IPC mappings) per device ordinal.  A
+ *    plan is sized for the SM count of the device current at csv_plan_create.
+ *    The only cross-device access is the STORE side of kv_handoff_direct into a
+ *    peer-mapped pool.
+ *  - Block ids handed to kernels (d_block_ids, d_block_tables) are NOT
+ *    range-checked on the device: an id outside [0, num_blocks) among the
+ *    entries a call addresses is undefined behaviour (an out-of-bounds access).
+ *    Entries a call does not address (past ceil(kv_len / 16)) are never read.
+ *    Ids that crossed a process boundary must be validated by the receiver
+ *    before the launch (replicas.PeerPools.push does).
  *
  * Pool layout (one pool = one decoder's, or the prefiller's, KV memory)
  *
@@ -266,16 +282,21 @@ int kv_append_tokens(kv_pool_t* dst, const csv_plan_t* plan, const void* d_k_new
 size_t csv_plan_workspace_bytes(const csv_attn_shape* shape, const int32_t* h_q_lens,
                                 const int32_t* h_kv_lens, int32_t batch, int32_t max_partition_tokens);
 /* Builds the plan and enqueues the copy of its work lists into d_workspace
- * (128-byte aligned) on `stream`.  q_len[b] must be in [0, kv_len[b]];
- * q_len = 0 rows are inert.  The plan may be used on that stream (or after
+ * (128-byte aligned) on `stream`.  q_len[b] must be in [0, kv_len[b]]
+ * (a row's own K/V is already counted in kv_len), with one exception: a decode
+ * row on an EMPTY cache, q_len = 1 and kv_len = 0, is accepted and gives
+ * O = 0, LSE = -inf (kv_append_tokens / the fused steps write nothing for it).
+ * Any other q_len > kv_len -> CSV_E_INVAL.  q_len = 0 rows are inert.  The plan may be used on that stream (or after
  * synchronising with it) until destroyed; the workspace must outlive it.
  * Launches of the SAME call on one plan share workspace (the decode partials;
  * the append partials and the append kernel's work queue): they must be
  * ordered on the device (same stream, or events), never concurrent.  A decode
  * call and an append call of one plan use disjoint regions and may overlap.
  * One plan serves all the layers of a step in turn.
- * d_workspace = NULL builds a host-only plan (no CUDA call): good for
- * csv_plan_info / csv_plan_*_items, refused (CSV_E_INVAL) by the attention calls.
+ * d_workspace = NULL builds a host-only plan (no device memory is touched; the
+ * only CUDA runtime call is the SM-count query of the current device, 148 being
+ * assumed when there is none): good for csv_plan_info / csv_plan_*_items,
+ * refused (CSV_E_INVAL) by the attention calls.
  * ws_bytes too small -> CSV_E_NOMEM. */
 int csv_plan_create(const csv_attn_shape* shape, const int32_t* h_q_lens, const int32_t* h_kv_lens,
                     int32_t batch, int32_t max_partition_tokens, void* d_workspace, size_t ws_bytes,
@@ -308,7 +329,7 @@ int32_t csv_plan_append_items(const csv_plan_t* plan, int32_t* h_out, int32_t ma
  *     s_j = q . K_j / sqrt(d),  j in [0, kv_len[b])
  *     O   = sum_j softmax(s)_j V_j          (bf16, round-to-nearest-even)
  *     LSE = ln sum_j exp(s_j)               (fp32, natural log)
- * kv_len = 0 -> O = 0, LSE = -inf.  bf16 inputs, fp32 scores / softmax /
+ * kv_len = 0 (empty cache) -> O = 0 (all bits zero), LSE = -inf.  bf16 inputs, fp32 scores / softmax /
  * accumulation; softmax weights are rounded to bf16 for the PV product.
  *
  * d_q:   [total_q][Hq][d] bf16, 16-byte aligned, total_q = sum of ALL q_lens of the plan in

@@ -56,18 +56,5 @@ def build_library(force=False, verbose=False):
     return LIB
 
 
-def build_microbench():
-    """csrc/bench_mma_rate.cu -> paper_2606_01839_b200/bench_mma_rate (stand-alone executable, not part of the library)."""
-    exe = os.path.join(os.path.dirname(LIB), "bench_mma_rate")
-    src = os.path.join(CSRC, "bench_mma_rate.cu")
-    if _stale(exe, [src] + [os.path.join(CSRC, h) for h in HEADERS]):
-        r = subprocess.run([NVCC] + FLAGS + ["-o", exe, src], capture_output=True, text=True)
-        if r.returncode != 0:
-            raise RuntimeError("nvcc failed on bench_mma_rate.cu:\n%s\n%s" % (r.stdout, r.stderr))
-    return exe
-
-
 if __name__ == "__main__":
     print(build_library(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
-    if "--microbench" in sys.argv:
-        print(build_microbench())

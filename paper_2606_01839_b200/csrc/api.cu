@@ -2,6 +2,7 @@
 // validation, plan upload, launches, and the host-buffer tail step.  No kernels here.
 #include <string.h>
 
+#include <atomic>
 #include <new>
 #include <vector>
 
@@ -15,17 +16,21 @@ int csv_set_cuda_error(int err) {
 }
 
 int csv_query_num_sms() {
-    static int cached = -1;
-    if (cached > 0) return cached;
+    // per device: a process may drive several GPUs (conserve_kv.h "Devices")
+    static std::atomic<int> cached[64];
     int dev = 0, n = 0;
-    if (cudaGetDevice(&dev) == cudaSuccess &&
-        cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0) {
-        cached = n;
-        return n;
+    if (cudaGetDevice(&dev) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return 148;   // B200; lets the planner run on a box without a GPU (host tests, host-only plans)
     }
-    (void)cudaGetLastError();
-    cached = 148;   // B200; lets the planner run on a box without a GPU (host tests)
-    return cached;
+    const bool slot = dev >= 0 && dev < 64;
+    if (slot && (n = cached[dev].load(std::memory_order_relaxed)) > 0) return n;
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) {
+        (void)cudaGetLastError();
+        return 148;
+    }
+    if (slot) cached[dev].store(n, std::memory_order_relaxed);
+    return n;
 }
 
 static bool aligned(const void* p, size_t a) { return ((uintptr_t)p & (a - 1)) == 0; }
@@ -128,6 +133,7 @@ static cu_get_range_fn driver_get_range() {
 // exported pointers often share one cudaMalloc allocation (the caller's caching allocator), so opens are counted.
 struct ipc_region {
     uint8_t handle[CSV_IPC_HANDLE_BYTES];
+    int device;                 // the device that was current at the open: the mapping belongs to its context
     void* base;                 // what cudaIpcOpenMemHandle returned
     std::vector<void*> users;   // pointers csv_ipc_open handed out (base + offset), one per open
 };
@@ -150,8 +156,10 @@ int csv_ipc_export(const void* d_ptr, void* out_handle, uint64_t* out_offset) {
 
 int csv_ipc_open(const void* handle, uint64_t offset, void** out_d_ptr) {
     if (!handle || !out_d_ptr) return CSV_E_INVAL;
+    int dev = 0;
+    CSV_CUDA_TRY(cudaGetDevice(&dev));
     for (ipc_region& r : g_ipc) {
-        if (memcmp(r.handle, handle, CSV_IPC_HANDLE_BYTES) == 0) {
+        if (r.device == dev && memcmp(r.handle, handle, CSV_IPC_HANDLE_BYTES) == 0) {
             r.users.push_back((uint8_t*)r.base + offset);
             *out_d_ptr = r.users.back();
             return CSV_OK;
@@ -163,6 +171,7 @@ int csv_ipc_open(const void* handle, uint64_t offset, void** out_d_ptr) {
     CSV_CUDA_TRY(cudaIpcOpenMemHandle(&base, h, cudaIpcMemLazyEnablePeerAccess));
     ipc_region r;
     memcpy(r.handle, handle, CSV_IPC_HANDLE_BYTES);
+    r.device = dev;
     r.base = base;
     r.users.push_back((uint8_t*)base + offset);
     *out_d_ptr = r.users.back();
@@ -178,8 +187,14 @@ int csv_ipc_close(void* d_ptr) {
             u.erase(u.begin() + (long)k);
             if (u.empty()) {
                 void* base = g_ipc[i].base;
+                const int owner = g_ipc[i].device;
                 g_ipc.erase(g_ipc.begin() + (long)i);
-                CSV_CUDA_TRY(cudaIpcCloseMemHandle(base));
+                int cur = 0;
+                CSV_CUDA_TRY(cudaGetDevice(&cur));
+                if (cur != owner) CSV_CUDA_TRY(cudaSetDevice(owner));
+                const cudaError_t ce = cudaIpcCloseMemHandle(base);
+                if (cur != owner) CSV_CUDA_TRY(cudaSetDevice(cur));
+                if (ce != cudaSuccess) return csv_set_cuda_error((int)ce);
             }
             return CSV_OK;
         }

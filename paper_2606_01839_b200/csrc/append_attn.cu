@@ -303,11 +303,10 @@ template <int D>
 int launch_append_t(const csv_plan* plan, const AppendParams& p, cudaStream_t stream) {
     constexpr int TB = 16 * D * 2;
     const size_t smem = (size_t)kAppendStages * kStageBlocks * 2 * TB + kAppendStages * 8;
-    static bool attr_set = false;
-    if (!attr_set) {
-        CSV_CUDA_TRY(cudaFuncSetAttribute(append_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_set = true;
-    }
+    static PerDeviceOnce attr;
+    CSV_CUDA_TRY(once_per_device(attr, [&] {
+        return cudaFuncSetAttribute(append_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    }));
     const int cap = plan->num_sms * 2;
     const int grid = p.n_items < cap ? p.n_items : cap;
     append_kernel<D><<<grid, kAppendWarps * 32, smem, stream>>>(p);

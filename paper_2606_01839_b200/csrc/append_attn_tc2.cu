@@ -13,6 +13,9 @@
 //              against 957 TFLOP/s): S_t = Q_t K^T (SS, M=128, N=64), O_t += P_t V (A = P from TMEM)
 // TMEM (all 512 columns): tile t at t*256: S/P buffer 0 [0,64), buffer 1 [64,128), O [128,256).
 #include <math.h>
+#include <stdlib.h>
+
+#include <algorithm>
 
 #include "common.cuh"
 #include "internal.h"
@@ -23,7 +26,6 @@ namespace {
 constexpr int kT2Threads = 352;
 constexpr int kChunk = 64;                 // KV tokens per pipeline step
 constexpr int kChunkBlocks = kChunk / 16;
-constexpr int kKSt = 4, kVSt = 4;          // ring depths (16 KiB stages)
 constexpr uint32_t kTmemCols2 = 512;
 
 struct AppendTc2Params {
@@ -42,13 +44,17 @@ struct AppendTc2Params {
 };
 
 constexpr uint32_t kOffQ2 = 0;                           // 2 tiles x [2 halves][128 rows][128 B]
-constexpr uint32_t kOffK2 = 65536;                       // kKSt x [2 halves][4 blocks][2048 B]
-constexpr uint32_t kOffV2 = kOffK2 + kKSt * 16384;       // kVSt x [4 blocks][4096 B]
-constexpr uint32_t kOffBar2 = kOffV2 + kVSt * 16384;     // mbarriers + TMEM slot
-constexpr uint32_t kSmemBytes2 = kOffBar2 + 256;
+constexpr uint32_t kOffK2 = 65536;                       // ST x [2 halves][4 blocks][2048 B]
+constexpr uint32_t smem_bytes2(int ST) { return kOffK2 + 2u * ST * 16384u + 256u; }
 
+// ST = depth of the K and V rings (16 KiB stages): 4 when the kernel has the SM to itself, 3 when the slim decode kernel
+// runs beside it (csv_tail_step)
+template <int ST>
 __global__ void __launch_bounds__(kT2Threads, 1) append_tc2_kernel(const __grid_constant__ AppendTc2Params p) {
     constexpr int D = 128;
+    constexpr int kKSt = ST, kVSt = ST;
+    constexpr uint32_t kOffV2 = kOffK2 + kKSt * 16384;       // kVSt x [4 blocks][4096 B]
+    constexpr uint32_t kOffBar2 = kOffV2 + kVSt * 16384;     // mbarriers + TMEM slot
     constexpr int TB = 4096;
     extern __shared__ __align__(1024) uint8_t smem[];
     const uint32_t sbase = smem_u32(smem);
@@ -405,13 +411,24 @@ int launch_append_attn_tc2(const csv_plan* plan, const kv_pool* pool, int layer,
     p.G = p.Hq / p.Hkv;
     p.scale_log2 = (float)(1.4426950408889634 / sqrt((double)s.head_dim));
     p.sched = reinterpret_cast<uint32_t*>(plan->d_ws + plan->lay.append_sched);
-    static bool attr_set = false;
-    if (!attr_set) {
-        CSV_CUDA_TRY(cudaFuncSetAttribute(append_tc2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes2));
-        attr_set = true;
+    int grid = p.n_items < plan->num_sms ? p.n_items : plan->num_sms;
+    if (const char* e = getenv("CSV_X_APPEND_GRID")) grid = std::max(1, std::min(grid, atoi(e)));   // experiment knob
+    // the work queue must start at zero whatever happened to an earlier launch on this plan
+    CSV_CUDA_TRY(cudaMemsetAsync(p.sched, 0, 8, (cudaStream_t)stream));
+    const char* e3 = getenv("CSV_X_APPEND_STAGES");
+    if (e3 && atoi(e3) == 3) {
+        static PerDeviceOnce attr3;
+        CSV_CUDA_TRY(once_per_device(attr3, [] {
+            return cudaFuncSetAttribute(append_tc2_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes2(3));
+        }));
+        append_tc2_kernel<3><<<grid, kT2Threads, smem_bytes2(3), (cudaStream_t)stream>>>(p);
+    } else {
+        static PerDeviceOnce attr4;
+        CSV_CUDA_TRY(once_per_device(attr4, [] {
+            return cudaFuncSetAttribute(append_tc2_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes2(4));
+        }));
+        append_tc2_kernel<4><<<grid, kT2Threads, smem_bytes2(4), (cudaStream_t)stream>>>(p);
     }
-    const int grid = p.n_items < plan->num_sms ? p.n_items : plan->num_sms;
-    append_tc2_kernel<<<grid, kT2Threads, kSmemBytes2, (cudaStream_t)stream>>>(p);
     CSV_CUDA_TRY(cudaGetLastError());
     return CSV_OK;
 }

@@ -3,11 +3,33 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <atomic>
+
 #define CSV_CUDA_TRY(expr)                                   \
     do {                                                     \
         cudaError_t e__ = (expr);                            \
         if (e__ != cudaSuccess) return csv_set_cuda_error((int)e__); \
     } while (0)
+
+// ---- per-device one-time setup ------------------------------------------------------------------
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) and the SM count belong to a DEVICE, not to the process: a process
+// that drives several GPUs (peer route of kv_handoff_direct) must repeat the setup on each.  One bit per device
+// ordinal; the setup is idempotent, so two threads racing on the first launch are harmless.
+struct PerDeviceOnce {
+    std::atomic<unsigned long long> mask{0};
+};
+template <typename F>
+static inline cudaError_t once_per_device(PerDeviceOnce& o, F&& setup) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64) return setup();
+    const unsigned long long bit = 1ull << dev;
+    if (o.mask.load(std::memory_order_acquire) & bit) return cudaSuccess;
+    e = setup();
+    if (e == cudaSuccess) o.mask.fetch_or(bit, std::memory_order_release);
+    return e;
+}
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 

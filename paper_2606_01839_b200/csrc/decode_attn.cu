@@ -80,16 +80,24 @@ __global__ void __launch_bounds__(128) decode_merge_kernel(const MergeGroup* __r
     if (lane == 0) lse[(size_t)g.q_start * Hq + (size_t)g.head * G + hh] = (M + log2f(L)) * 0.6931471805599453f;
 }
 
-template <int D, int STAGES>
-__global__ void __launch_bounds__(kDecodeWarps * 32, 1) decode_kernel(const __grid_constant__ DecodeParams p) {
+// Decode rows on an empty cache (q_len = 1, kv_len = 0): O = 0, LSE = -inf.  One CTA per row.
+__global__ void decode_zero_rows_kernel(const int32_t* __restrict__ rows, int row_elems, int Hq, uint16_t* out, float* lse) {
+    const int32_t r = rows[blockIdx.x];   // plan data
+    pdl_wait();
+    for (int i = threadIdx.x; i < row_elems / 2; i += blockDim.x) reinterpret_cast<uint32_t*>(out + (size_t)r * row_elems)[i] = 0u;
+    for (int h = threadIdx.x; h < Hq; h += blockDim.x) lse[(size_t)r * Hq + h] = -INFINITY;
+}
+
+template <int D, int STAGES, int WARPS>
+__global__ void __launch_bounds__(WARPS * 32, WARPS == 8 ? 1 : 512 / (WARPS * 32)) decode_kernel(const __grid_constant__ DecodeParams p) {
     constexpr int TB = 16 * D * 2;   // tile bytes
     constexpr int KS = D / 16;       // k-steps of Q K^T
     constexpr int NT = D / 8;        // n-tiles of P V
     extern __shared__ __align__(1024) uint8_t smem[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int worker = blockIdx.x * kDecodeWarps + warp;
+    const int worker = blockIdx.x * WARPS + warp;
     uint8_t* ring = smem + (size_t)warp * STAGES * 2 * TB;
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)kDecodeWarps * STAGES * 2 * TB) + warp * STAGES;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)WARPS * STAGES * 2 * TB) + warp * STAGES;
     if (lane == 0) {
         for (int s = 0; s < STAGES; ++s) mbar_init(&bars[s], 1);
         fence_mbar_init();
@@ -294,16 +302,15 @@ __global__ void __launch_bounds__(kDecodeWarps * 32, 1) decode_kernel(const __gr
     }
 }
 
-template <int D, int STAGES>
+template <int D, int STAGES, int WARPS>
 int launch_decode_t(const csv_plan* plan, const DecodeParams& p, cudaStream_t stream) {
     constexpr int TB = 16 * D * 2;
-    const size_t smem = (size_t)kDecodeWarps * STAGES * 2 * TB + (size_t)kDecodeWarps * STAGES * 8;
-    static bool attr_set = false;
-    if (!attr_set) {
-        CSV_CUDA_TRY(cudaFuncSetAttribute(decode_kernel<D, STAGES>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_set = true;
-    }
-    CSV_CUDA_TRY(launch_pdl(decode_kernel<D, STAGES>, dim3(plan->decode_grid), dim3(kDecodeWarps * 32), smem, stream, p));
+    const size_t smem = (size_t)WARPS * STAGES * 2 * TB + (size_t)WARPS * STAGES * 8;
+    static PerDeviceOnce attr;
+    CSV_CUDA_TRY(once_per_device(attr, [&] {
+        return cudaFuncSetAttribute(decode_kernel<D, STAGES, WARPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    }));
+    CSV_CUDA_TRY(launch_pdl(decode_kernel<D, STAGES, WARPS>, dim3(plan->decode_grid), dim3(WARPS * 32), smem, stream, p));
     const int ng = (int)plan->decode_groups.size();
     if (ng > 0) {
         const int warps = ng * p.G;
@@ -318,8 +325,12 @@ int launch_decode_t(const csv_plan* plan, const DecodeParams& p, cudaStream_t st
 
 int launch_decode(const csv_plan* plan, const kv_pool* pool, int layer, const void* q, const int32_t* tables,
                   int max_blocks, void* out, float* lse, void* stream, const void* k_new, const void* v_new) {
-    if (plan->decode_items.empty()) return CSV_OK;
     const kv_pool_desc& s = pool->desc;
+    if (!plan->zero_rows.empty())
+        CSV_CUDA_TRY(launch_pdl(decode_zero_rows_kernel, dim3((unsigned)plan->zero_rows.size()), dim3(128), 0, (cudaStream_t)stream,
+                                reinterpret_cast<const int32_t*>(plan->d_ws + plan->lay.zero_rows),
+                                plan->shape.num_q_heads * s.head_dim, plan->shape.num_q_heads, (uint16_t*)out, lse));
+    if (plan->decode_items.empty()) return CSV_OK;
     DecodeParams p;
     p.items = reinterpret_cast<const DecodeItem*>(plan->d_ws + plan->lay.decode_items);
     p.worker_begin = reinterpret_cast<const int32_t*>(plan->d_ws + plan->lay.worker_begin);
@@ -338,6 +349,9 @@ int launch_decode(const csv_plan* plan, const kv_pool* pool, int layer, const vo
     p.Hkv = plan->shape.num_kv_heads;
     p.G = p.Hq / p.Hkv;
     p.scale_log2 = (float)(1.4426950408889634 / sqrt((double)s.head_dim));
-    if (s.head_dim == 128) return launch_decode_t<128, 3>(plan, p, (cudaStream_t)stream);
-    return launch_decode_t<64, 6>(plan, p, (cudaStream_t)stream);
+    if (s.head_dim == 128) {
+        if (plan->decode_warps == 2) return launch_decode_t<128, 4, 2>(plan, p, (cudaStream_t)stream);
+        return launch_decode_t<128, 3, 8>(plan, p, (cudaStream_t)stream);
+    }
+    return launch_decode_t<64, 6, 8>(plan, p, (cudaStream_t)stream);
 }

@@ -230,6 +230,7 @@ __global__ void __launch_bounds__(kThreads) append_tokens_kernel(uint8_t* pool, 
             if (q_start[mid] <= row) lo = mid; else hi = mid;
         }
         const int pos = kv_len[lo] - q_len[lo] + (row - q_start[lo]);
+        if (pos < 0) continue;   // decode row on an empty cache (q_len 1, kv_len 0): it has no position to write
         const int block = __ldg(tables + (size_t)lo * max_blocks + (pos >> 4));
         const int slot = pos & 15;
         const uint8_t* src = (kv ? v_new : k_new) + (((size_t)layer * total_q + row) * Hkv + head) * D * 2 + chunk * 16;

@@ -75,6 +75,7 @@ constexpr int kAppendKvSplit = 8192; // default KV tokens per append partition
 struct PlanLayout {   // byte offsets into the caller's workspace (all 128-byte aligned)
     size_t decode_items, worker_begin, decode_groups, decode_po, decode_pml;
     size_t append_items, append_groups, append_po, append_pml;
+    size_t zero_rows;   // int32 rows of d_out / d_lse whose conversation has q_len = 1 and an empty cache
     size_t conv_meta;   // int32 [q_start[batch+1] | kv_len[batch] | q_len[batch]]
     size_t append_sched;   // uint32 [next item, CTAs done]: the append kernel's work queue, zero between launches
     size_t total;
@@ -83,7 +84,7 @@ struct PlanLayout {   // byte offsets into the caller's workspace (all 128-byte 
 struct csv_plan {
     csv_attn_shape shape;
     int32_t batch;
-    int32_t max_partition_tokens;        // decode partition cap in force (default 2048)
+    int32_t max_partition_tokens;        // decode partition cap in force (1 << 30 when the caller passed 0: share cuts only)
     int32_t max_partition_tokens_user;   // what the caller passed (0 = defaults)
     int32_t num_sms;
     std::vector<int32_t> q_lens, kv_lens, q_start;
@@ -94,7 +95,9 @@ struct csv_plan {
     std::vector<MergeGroup> decode_groups;   // groups with count > 1 only
     int32_t n_decode_rows;
     int32_t decode_grid;                     // CTAs
+    int32_t decode_warps;                    // warp-workers per CTA (8; 2 = the slim kernel that runs beside the append CTAs)
     int32_t n_decode_partials;               // partial slots (non-direct items)
+    std::vector<int32_t> zero_rows;          // q rows of decode conversations with kv_len = 0 (O = 0, LSE = -inf)
     // append
     std::vector<AppendItem> append_items;
     std::vector<MergeGroup> append_groups;   // groups with count > 1 only

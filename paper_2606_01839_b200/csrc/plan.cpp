@@ -13,6 +13,8 @@
 // its 8 KV heads spans ~9.25 shares.
 // The schedule depends only on the lengths: results are bit-identical under any block
 // permutation and from run to run.
+#include <stdlib.h>
+
 #include <algorithm>
 #include <new>
 
@@ -37,15 +39,19 @@ static void plan_decode(csv_plan* p) {
     const int part_blocks = std::max(1, p->max_partition_tokens / CSV_BLOCK_SIZE);
     int64_t units = 0;
     p->n_decode_rows = 0;
+    p->zero_rows.clear();
     for (int b = 0; b < p->batch; ++b)
         if (p->q_lens[b] == 1) {
             units += (int64_t)((p->kv_lens[b] + CSV_BLOCK_SIZE - 1) / CSV_BLOCK_SIZE) * Hkv;
             ++p->n_decode_rows;
+            if (p->kv_lens[b] == 0) p->zero_rows.push_back(p->q_start[(size_t)b]);   // empty cache: O = 0, LSE = -inf
         }
     // CTAs: one per SM, fewer when there is under 4 blocks of work per warp
-    int64_t want = (units + (int64_t)kDecodeWarps * 4 - 1) / ((int64_t)kDecodeWarps * 4);
+    const int WPC = p->decode_warps;   // warp-workers per CTA
+    int64_t want = (units + (int64_t)WPC * 4 - 1) / ((int64_t)WPC * 4);
     p->decode_grid = (int)std::max<int64_t>(1, std::min<int64_t>(p->num_sms, want));
-    const int64_t W = (int64_t)p->decode_grid * kDecodeWarps;
+    if (const char* e = getenv("CSV_X_DECODE_GRID")) p->decode_grid = std::max(1, std::min(p->decode_grid, atoi(e)));   // experiment knob
+    const int64_t W = (int64_t)p->decode_grid * WPC;
     p->worker_begin.assign((size_t)W + 1, 0);
     p->decode_items.clear();
     p->decode_items.reserve((size_t)W + (size_t)p->n_decode_rows * Hkv + 16);
@@ -64,7 +70,7 @@ static void plan_decode(csv_plan* p) {
         ++next_start;
     }
     for (int b = 0; b < p->batch; ++b) {
-        if (p->q_lens[b] != 1) continue;
+        if (p->q_lens[b] != 1 || p->kv_lens[b] == 0) continue;
         const int nblk = (p->kv_lens[b] + CSV_BLOCK_SIZE - 1) / CSV_BLOCK_SIZE;
         for (int g = 0; g < Hkv; ++g) {
             const size_t first_item = p->decode_items.size();
@@ -220,6 +226,7 @@ static void plan_layout(csv_plan* p) {
     L.decode_groups = take(p->decode_groups.size() * sizeof(MergeGroup));
     L.append_items = take(p->append_items.size() * sizeof(AppendItem));
     L.append_groups = take(p->append_groups.size() * sizeof(MergeGroup));
+    L.zero_rows = take(p->zero_rows.size() * sizeof(int32_t));
     L.append_sched = take(128);   // zero in the uploaded image; the kernel's last CTA zeroes it again
     std::vector<int32_t> meta;
     meta.insert(meta.end(), p->q_start.begin(), p->q_start.end());
@@ -242,6 +249,7 @@ static void plan_layout(csv_plan* p) {
     put(L.append_items, p->append_items.data(), p->append_items.size() * sizeof(AppendItem));
     put(L.append_groups, p->append_groups.data(), p->append_groups.size() * sizeof(MergeGroup));
     put(L.conv_meta, meta.data(), meta.size() * sizeof(int32_t));
+    put(L.zero_rows, p->zero_rows.data(), p->zero_rows.size() * sizeof(int32_t));
 }
 
 // Builds the host side of a plan.  Returns NULL on bad arguments.
@@ -252,7 +260,10 @@ csv_plan* csv_plan_build_host(const csv_attn_shape* shape, const int32_t* h_q_le
     if (max_partition_tokens < 0 || max_partition_tokens % CSV_BLOCK_SIZE != 0) return nullptr;
     int64_t total_q = 0;
     for (int b = 0; b < batch; ++b) {
-        if (h_kv_lens[b] < 0 || h_q_lens[b] < 0 || h_q_lens[b] > h_kv_lens[b]) return nullptr;
+        // q_len <= kv_len (a row's own K/V is in the cache), except the decode row on an EMPTY cache (q_len 1, kv_len 0):
+        // nothing to attend to, O = 0 and LSE = -inf (conserve_kv.h a4)
+        if (h_kv_lens[b] < 0 || h_q_lens[b] < 0) return nullptr;
+        if (h_q_lens[b] > h_kv_lens[b] && !(h_q_lens[b] == 1 && h_kv_lens[b] == 0)) return nullptr;
         total_q += h_q_lens[b];
     }
     if (total_q > INT32_MAX) return nullptr;
@@ -272,6 +283,8 @@ csv_plan* csv_plan_build_host(const csv_attn_shape* shape, const int32_t* h_q_le
     for (int b = 0; b < batch; ++b) p->q_start[(size_t)b + 1] = p->q_start[(size_t)b] + h_q_lens[b];
     p->total_q = (int32_t)total_q;
     p->d_ws = nullptr;
+    p->decode_warps = kDecodeWarps;
+    if (const char* e = getenv("CSV_X_DECODE_WARPS")) p->decode_warps = atoi(e) == 2 ? 2 : kDecodeWarps;   // experiment knob
     plan_decode(p);
     plan_append(p);
     plan_layout(p);

@@ -67,7 +67,7 @@ __device__ __forceinline__ void mma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_
 // Single-thread forms taking the descriptor as (lo, hi) words: the caller builds the descriptor once and adds
 // (byte offset >> 4) to the low word per MMA (the start-address field is its low 14 bits).  With the base words made
 // warp-uniform (a shuffle broadcast tells the compiler) the per-MMA words are formed by UIADD3 on the uniform datapath.
-// Rates measured with csrc/bench_mma_rate.cu (one thread issuing back to back, one CTA per SM): M128 N64 K16 SS 48-60
+// Rates measured in round 1 (profiles/r1_mma_rate.txt: one thread issuing back to back, one CTA per SM): M128 N64 K16 SS 48-60
 // cycles per MMA (it fetches 6 KiB of shared-memory operands at 128 B/clk; its math is 32 cycles), N128 SS 64, N128 TS
 // 64, N256 SS 128.
 __device__ __forceinline__ void mma_ss_lohi(uint32_t d_tmem, uint32_t a_lo, uint32_t a_hi, uint32_t b_lo, uint32_t b_hi,

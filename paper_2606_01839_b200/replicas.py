@@ -13,23 +13,26 @@ def rank_seed(base_seed, rank):
     return int(base_seed) + 100 * int(rank)
 
 
-def bind_conversations(need_blocks, pool_blocks, world):
-    """The paper's placement rule across `world` decoders, host-only replay:
-    each arriving conversation goes to the decoder with the lowest active occupancy that fits.
-    Returns the decoder index per conversation (-1 = nobody fits)."""
-    used = [0] * world
-    out = []
+def bind_conversations(need_blocks, pools):
+    """Replay of an arrival sequence through the library's placement call: each arriving
+    conversation is bound by csv_place to one of `pools` (binding.KvPool handles, one per decoder) and its blocks are
+    allocated there, for life.  Returns (decoder index per conversation, -1 = nobody fits; block ids per conversation).
+    No placement arithmetic here: the rule lives in csv_place."""
+    from . import binding as B
+
+    where, tables = [], []
     for need in need_blocks:
-        best = -1
-        for r in range(world):
-            if pool_blocks - used[r] < need:
-                continue
-            if best < 0 or used[r] < used[best]:
-                best = r
-        if best >= 0:
-            used[best] += int(need)
-        out.append(best)
-    return out
+        try:
+            k = B.csv_place(pools, int(need))
+        except B.CsvError as e:
+            if e.code != B.CSV_E_NOMEM:
+                raise
+            where.append(-1)
+            tables.append(None)
+            continue
+        where.append(k)
+        tables.append(pools[k].alloc_blocks(int(need)))
+    return where, tables
 
 
 def aggregate(dist, local_ms, local_units, device="cpu"):
@@ -90,7 +93,11 @@ class PeerPools:
 
         key = (ticket["decoder"], ticket["handle"], ticket["offset"])
         if key not in self._pools:
-            NL, nb, Hkv, d = ticket["shape"]
+            NL, nb, Hkv, d = (int(x) for x in ticket["shape"])
+            if local_pool is not None:      # the ticket's shape is only trusted as far as it matches what we hold
+                ld = local_pool.desc
+                if (ld.num_layers, ld.num_blocks, ld.num_kv_heads, ld.head_dim) != (NL, nb, Hkv, d):
+                    raise ValueError("ticket shape does not match the local pool")
             desc = B.pool_desc(NL, nb, Hkv, d)
             if ticket["handle"] is None:
                 if local_pool is None:
@@ -108,6 +115,14 @@ class PeerPools:
         from . import binding as B
 
         pool = self.get(ticket, local_pool)
+        # The ids came over a channel and the kernel does not range-check them (conserve_kv.h): one bad id would be a
+        # silent out-of-bounds write into another process's allocation.  Validate on the host before launching.
+        ids, nb = ticket["ids"], ticket["shape"][1]
+        need = (ticket["token_offset"] + ticket["tokens"] + 15) // 16
+        if ticket["tokens"] <= 0 or ticket["token_offset"] < 0 or len(ids) < need:
+            raise ValueError("ticket: table shorter than ceil((offset + tokens) / 16)")
+        if any((not isinstance(i, int)) or i < 0 or i >= nb for i in ids) or len(set(ids)) != len(ids):
+            raise ValueError("ticket: block ids must be unique and inside [0, num_blocks)")
         if d_ids is None:
             d_ids = torch.tensor(ticket["ids"], dtype=torch.int32, device="cuda")
         B.kv_handoff_direct(pool, d_k, d_v, ticket["tokens"], ticket["token_offset"], d_ids, len(ticket["ids"]), stream)

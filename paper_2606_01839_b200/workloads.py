@@ -108,17 +108,15 @@ class TailWorkload:
         B.append_prefill_attn(self.plan, self.pool, layer, self.d_q, self.d_tables, self.max_blocks, self.d_out,
                               self.d_lse, stream)
 
-    def logical_kv(self, oracle, b, layer=0):
-        """Copy conversation b's blocks back and let the ORACLE gather them (paged -> logical)."""
+    def conversation_blocks_host(self, b, layer=0):
+        """Conversation b's blocks of one layer copied back to the host as a compact uint16 image
+        [len(table)][2][Hkv][16][d] in table order (raw pool bytes: whoever reads them applies the layout)."""
         ids = self.tables[b]
         per_block = 2 * self.Hkv * 16 * self.d                       # int16 elements of one (layer, block)
         base = layer * self.num_blocks * per_block
         idx = torch.from_numpy(ids.astype(np.int64)).cuda()
         blocks = self.d_pool[base:base + self.num_blocks * per_block].view(self.num_blocks, per_block)[idx]
-        img = blocks.cpu().contiguous().numpy().view(np.uint16).reshape(-1)
-        # a compact 1-layer pool holding only this conversation's blocks, identity table
-        K, V = oracle.gather(img, len(ids), self.Hkv, self.d, 0, np.arange(len(ids), dtype=np.int32), self.kv_lens[b])
-        return K, V
+        return blocks.cpu().contiguous().numpy().view(np.uint16).reshape(-1)
 
 
 def config_tail_workload(k, seed=None, layers=None, mpt=0, v_mean=0.0):

@@ -3,6 +3,8 @@
 Inputs are built on the host with numpy + the ORACLE's layout restatement (oracle.scatter)
 and uploaded; the CUDA path never produces an oracle input or an expected value.
 """
+import os
+
 import numpy as np
 import torch
 
@@ -117,15 +119,29 @@ def oracle_attention(sc, q_lens, q_bits, layer=0):
     return O, LSE
 
 
+def logical_kv(oracle, wl, b, layer=0):
+    """Conversation b of a device workload as logical K, V: its blocks are copied back as raw pool bytes and the
+    ORACLE gathers them (paged -> logical) from a compact 1-layer pool with the identity table."""
+    img = wl.conversation_blocks_host(b, layer)
+    n = len(wl.tables[b])
+    return oracle.gather(img, n, wl.Hkv, wl.d, 0, np.arange(n, dtype=np.int32), wl.kv_lens[b])
+
+
 def assert_close(O, LSE, O_ref, LSE_ref, what="", norm=True):
     assert np.all(np.isfinite(O)), "%s: non-finite O" % what
     assert np.all(np.isfinite(LSE)), "%s: non-finite LSE" % what
     err = np.abs(O - O_ref)
-    # north_star's absolute bound is stated for "outputs O(1)": a bf16 output near 3 already rounds by 2^-7 = 7.8e-3.
-    # Rows whose reference exceeds 1 in magnitude (a handful of visible keys) get the same bound relative to |O|_inf.
-    scale = np.maximum(1.0, np.abs(O_ref).max(axis=-1, keepdims=True))
-    worst = (err / scale).max()
-    assert worst <= O_TOL, "%s: max |O err| %.3e (scaled %.3e) > %.0e" % (what, err.max(), worst, O_TOL)
+    # north_star's 1e-2 absolute bound is stated for "outputs O(1)".  A bf16 output of magnitude in [2^k, 2^(k+1)) is
+    # rounded by up to half an ulp = 2^(k-8) on its own (7.8e-3 in [2,4), 1.6e-2 in [4,8)), so from |O_ref| >= 2 on that
+    # half-ulp is added to the bound, element by element; below 2 the bound is the plain 1e-2 (DESIGN.md S20).
+    mag = np.abs(O_ref)
+    extra = np.where(mag >= 2.0, np.exp2(np.floor(np.log2(np.maximum(mag, 1.0))) - 8.0), 0.0)
+    bad = err > O_TOL + extra
+    assert not bad.any(), "%s: max |O err| %.3e > %.0e (+ half a bf16 ulp where |O_ref| >= 2); worst excess %.3e" % (
+        what, err.max(), O_TOL, (err - O_TOL - extra).max())
+    if (err > O_TOL).any() and os.environ.get("CSV_TOL_LOG"):   # which cases needed the half-ulp term (listed in S20)
+        with open(os.environ["CSV_TOL_LOG"], "a") as f:
+            f.write("%s: max err %.4e at |O_ref| %.3f\n" % (what, err.max(), float(mag.reshape(-1)[err.argmax()])))
     lerr = np.abs(LSE - LSE_ref).max()
     assert lerr <= LSE_TOL, "%s: max |LSE err| %.3e > %.0e" % (what, lerr, LSE_TOL)
     if norm:

@@ -139,6 +139,55 @@ def test_decode_tolerates_aliased_blocks(oracle):
     assert_close(O, LSE, *oracle_attention(sc, [1, 1], q), what="aliased")
 
 
+def test_decode_row_on_an_empty_cache_gives_zero_and_minus_infinity(oracle):
+    # conserve_kv.h a4 / SURVEY §8b: kv_len = 0 -> O = 0, LSE = -inf (the oracle's O1 step 6), next to ordinary rows
+    for Hq, Hkv, d in ((32, 8, 128), (4, 1, 64)):
+        rng = np.random.default_rng(77)
+        kv = [0, 40, 0, 300, 0]
+        sc = Scenario(oracle, rng, Hq, Hkv, d, kv, poison=True).commit().upload()
+        q = synth.normal_bf16(rng, (len(kv), Hq, d))
+        O, LSE, info = run_attention(sc, [1] * len(kv), q, which="decode")
+        assert info["n_decode_rows"] == len(kv)
+        for b, t in enumerate(kv):
+            o_ref, l_ref = oracle.attention(q[b:b + 1], sc.K[b][0][:t], sc.V[b][0][:t])
+            if t == 0:
+                assert np.all(o_ref == 0.0) and np.all(np.isneginf(l_ref))          # what the oracle says
+                assert np.all(O[b] == 0.0) and np.all(np.isneginf(LSE[b])), "empty-cache row %d" % b
+            else:
+                assert_close(O[b:b + 1], LSE[b:b + 1], o_ref, l_ref, what="row %d beside empty-cache rows" % b)
+        # the fused step writes nothing for an empty-cache row and the pool stays as it was
+        shape = B.attn_shape(Hq, Hkv, d)
+        ws = torch.empty(B.csv_plan_workspace_bytes(shape, [1], [0]), dtype=torch.uint8, device="cuda")
+        plan = B.Plan(shape, [1], [0], 0, ws)
+        before = sc.d_image.clone()
+        d_out = torch.full((1, Hq, d), 0x7FC0, dtype=torch.int16, device="cuda")
+        d_lse = torch.zeros((1, Hq), dtype=torch.float32, device="cuda")
+        kn = torch.ones(Hkv * d, dtype=torch.int16, device="cuda")
+        B.paged_decode_step(plan, sc.pool, 0, torch.zeros(Hq * d, dtype=torch.int16, device="cuda"), kn, kn, sc.d_tables,
+                            sc.max_blocks, d_out, d_lse)
+        B.kv_append_tokens(sc.pool, plan, kn, kn, sc.d_tables, sc.max_blocks)
+        torch.cuda.synchronize()
+        assert torch.equal(before, sc.d_image) and bool((d_out == 0).all()) and bool(torch.isneginf(d_lse).all())
+
+
+def test_decode_on_every_visible_device(oracle):
+    # Per-device library state (kernel attributes, SM count): a decode must work on each device in turn inside one
+    # process.  On a 1-GPU box this is a set_device round trip followed by a launch; with more GPUs every one runs.
+    n = torch.cuda.device_count()
+    cur = torch.cuda.current_device()
+    try:
+        for dev in list(range(n)) + [0]:
+            torch.cuda.set_device(dev)
+            with torch.cuda.device(dev):
+                rng = np.random.default_rng(5 + dev)
+                sc = Scenario(oracle, rng, 32, 8, 128, [70, 1000]).commit().upload()
+                q = synth.normal_bf16(rng, (3, 32, 128))
+                O, LSE, _ = run_attention(sc, [1, 2], q)          # decode kernel + tcgen05 append kernel
+                assert_close(O, LSE, *oracle_attention(sc, [1, 2], q), what="device %d" % dev)
+    finally:
+        torch.cuda.set_device(cur)
+
+
 def test_attention_argument_errors(oracle):
     rng = np.random.default_rng(42)
     sc = Scenario(oracle, rng, 32, 8, 128, [100]).commit().upload()

@@ -9,7 +9,7 @@ import torch
 
 from paper_2606_01839_b200 import binding as B
 from paper_2606_01839_b200 import synth, workloads
-from harness import assert_close, bf16_dev_to_f64, dev_to_u16
+from harness import assert_close, bf16_dev_to_f64, dev_to_u16, logical_kv
 
 pytestmark = pytest.mark.gpu
 
@@ -25,7 +25,7 @@ def check_rows(oracle, wl, layer, samples, O, LSE, what):
     cache = {}
     for b, i in samples:
         if b not in cache:
-            cache = {b: wl.logical_kv(oracle, b, layer)}     # keep one conversation at a time (131k tokens = 512 MiB)
+            cache = {b: logical_kv(oracle, wl, b, layer)}     # keep one conversation at a time (131k tokens = 512 MiB)
         K, V = cache[b]
         m = wl.q_lens[b]
         n = wl.kv_lens[b] - m + i + 1                        # keys visible to row i (decode: m = 1, i = 0, n = kv_len)

@@ -174,7 +174,7 @@ def check_decode_plan(q_lens, kv_lens, Hq, Hkv, d, mpt=0):
         cover.setdefault((conv, head), []).append((b0, b1, partial, direct))
     rows = [b for b in range(len(q_lens)) if q_lens[b] == 1]
     assert info["n_decode_rows"] == len(rows)
-    assert set(cover) == {(b, g) for b in rows for g in range(Hkv)}
+    assert set(cover) == {(b, g) for b in rows for g in range(Hkv) if kv_lens[b] > 0}   # an empty cache has no blocks
     seen_partials = set()
     for (conv, head), parts in cover.items():
         assert parts[0][0] == 0 and parts[-1][1] == (kv_lens[conv] + 15) // 16
@@ -220,6 +220,12 @@ def test_decode_plan_edge_lengths_and_partition_sizes():
     assert info["n_decode_items"] == 0
     with pytest.raises(B.CsvError):
         B.Plan(B.attn_shape(32, 8, 128), [2], [1])            # q_len > kv_len
+    with pytest.raises(B.CsvError):
+        B.Plan(B.attn_shape(32, 8, 128), [2], [0])            # ... also on an empty cache, unless it is a decode row:
+    _, info = check_decode_plan([1, 1, 1], [0, 40, 0], 32, 8, 128)   # q_len 1, kv_len 0 -> O = 0, LSE = -inf (header a4)
+    assert info["n_decode_rows"] == 3 and info["n_decode_items"] >= 8
+    _, info = check_decode_plan([1], [0], 4, 1, 64)
+    assert info["n_decode_rows"] == 1 and info["n_decode_items"] == 0
     with pytest.raises(B.CsvError):
         B.Plan(B.attn_shape(32, 8, 128), [1], [10], 24)       # partition not a multiple of 16
     with pytest.raises(B.CsvError):

@@ -14,6 +14,9 @@ from paper_2606_01839_b200 import build as libbuild
 from paper_2606_01839_b200 import replicas, synth
 
 
+FAKE = 1 << 40          # a 128-byte aligned "device" address: the allocator and tickets are host-only
+
+
 def _worker(rank, world, port, ret):
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
     dist.init_process_group("gloo", rank=rank, world_size=world)
@@ -45,14 +48,21 @@ def test_two_replicas_share_nothing_but_the_clock():
 
 
 def test_placement_replay_balances_decoders():
-    # lowest active occupancy wins; a full decoder is skipped
+    # lowest active occupancy wins; a full decoder is skipped.  The replay goes through
+    # csv_place / kv_alloc_blocks on real pool handles (host-only pools over a fake device address).
     need = [10, 10, 10, 30, 5, 5, 100, 1]
-    got = replicas.bind_conversations(need, pool_blocks=60, world=2)
-    assert got == [0, 1, 0, 1, 0, 0, -1, 0]
+    pools = [B.KvPool(B.pool_desc(1, 60, 8, 128), FAKE, 1 << 40) for _ in range(2)]
+    where, tables = replicas.bind_conversations(need, pools)
+    assert where == [0, 1, 0, 1, 0, 0, -1, 0]
+    assert [None if t is None else len(t) for t in tables] == [10, 10, 10, 30, 5, 5, None, 1]
+    assert [p.used_blocks for p in pools] == [31, 40]
+    # unequal decoders: occupancy is the RATIO used / total (S17), not the block count
+    pools = [B.KvPool(B.pool_desc(1, 100, 8, 128), FAKE, 1 << 40), B.KvPool(B.pool_desc(1, 20, 8, 128), FAKE, 1 << 40)]
+    where, _ = replicas.bind_conversations([10, 1, 1, 1], pools)
+    assert where == [0, 1, 1, 0]            # 10/100 vs 0/20 -> 1; 10 % vs 5 % -> 1; 10 % vs 10 % tie -> 0
     assert replicas.aggregate(None, 1.5, 7.0) == (1.5, 7.0)
 
 
-FAKE = 1 << 40          # a 128-byte aligned "device" address: the allocator and tickets are host-only
 
 
 def _handoff_worker(rank, world, port, ret):
