@@ -56,7 +56,9 @@ static double bf16_to_double(uint16_t bits) {
  */
 int orc_attention(const uint16_t* q, const uint16_t* K, const uint16_t* V, int R, int L, int Hq, int Hkv,
                   int d, double* O, double* LSE) {
-    if (R < 0 || L < 0 || R > L || Hq <= 0 || Hkv <= 0 || d <= 0 || Hq % Hkv != 0) return -1;
+    /* R <= L (a row's own key is in the cache), except the one decode row on an EMPTY cache (R = 1, L = 0, so P = -1 and
+     * n = 0): SURVEY 8c O1 step 6 / conserve_kv.h a4, O = 0 and LSE = -inf. */
+    if (R < 0 || L < 0 || (R > L && !(R == 1 && L == 0)) || Hq <= 0 || Hkv <= 0 || d <= 0 || Hq % Hkv != 0) return -1;
     const int G = Hq / Hkv;
     const int P = L - R;
     const double inv_sqrt_d = 1.0 / sqrt((double)d);

@@ -119,6 +119,22 @@ def oracle_attention(sc, q_lens, q_bits, layer=0):
     return O, LSE
 
 
+def oracle_abs_weighted(sc, q_lens, q_bits, layer=0):
+    """A[r][h][c] = sum_j p_j |V_j[c]|: the oracle's O1 run on |V| (sign bit of every bf16 cleared).  It is what the two
+    bf16 roundings of the GPU path (P before the PV product, O on output) are relative to (S20)."""
+    total_q = int(np.sum(q_lens))
+    A = np.zeros((total_q, sc.Hq, sc.d))
+    r = 0
+    for b, m in enumerate(q_lens):
+        if m == 0:
+            continue
+        L = sc.kv_lens[b]
+        if L > 0:
+            A[r:r + m] = sc.oracle.attention(q_bits[r:r + m], sc.K[b][layer][:L], sc.V[b][layer][:L] & np.uint16(0x7FFF))[0]
+        r += m
+    return A
+
+
 def logical_kv(oracle, wl, b, layer=0):
     """Conversation b of a device workload as logical K, V: its blocks are copied back as raw pool bytes and the
     ORACLE gathers them (paged -> logical) from a compact 1-layer pool with the identity table."""
@@ -127,7 +143,7 @@ def logical_kv(oracle, wl, b, layer=0):
     return oracle.gather(img, n, wl.Hkv, wl.d, 0, np.arange(n, dtype=np.int32), wl.kv_lens[b])
 
 
-def assert_close(O, LSE, O_ref, LSE_ref, what="", norm=True):
+def assert_close(O, LSE, O_ref, LSE_ref, what="", norm=True, A_ref=None):
     assert np.all(np.isfinite(O)), "%s: non-finite O" % what
     assert np.all(np.isfinite(LSE)), "%s: non-finite LSE" % what
     err = np.abs(O - O_ref)
@@ -136,10 +152,17 @@ def assert_close(O, LSE, O_ref, LSE_ref, what="", norm=True):
     # half-ulp is added to the bound, element by element; below 2 the bound is the plain 1e-2 (S20).
     mag = np.abs(O_ref)
     extra = np.where(mag >= 2.0, np.exp2(np.floor(np.log2(np.maximum(mag, 1.0))) - 8.0), 0.0)
-    bad = err > O_TOL + extra
-    assert not bad.any(), "%s: max |O err| %.3e > %.0e (+ half a bf16 ulp where |O_ref| >= 2); worst excess %.3e" % (
-        what, err.max(), O_TOL, (err - O_TOL - extra).max())
-    if (err > O_TOL).any() and os.environ.get("CSV_TOL_LOG"):   # which cases needed the half-ulp term (listed in S20)
+    tol = O_TOL + extra
+    if A_ref is not None:
+        # Only the q-scaled cases pass A_ref = sum_j p_j |V_j| (oracle_abs_weighted).  With scores of +-30 the softmax
+        # sits on one or two keys, so outputs reach |V|max ~ 4 and the rounding of P to bf16 (allowed: S7; unit roundoff
+        # 2^-8) is no longer averaged over many keys: |err| <= 2^-8 A (P) + 2^-8 |O| (output) <= 2^-7 A.  The bound is
+        # the larger of the plain gate and that one, element by element (S20).
+        tol = np.maximum(tol, np.exp2(-7.0) * A_ref)
+    bad = err > tol
+    assert not bad.any(), "%s: max |O err| %.3e > %.0e (+ half a bf16 ulp where |O_ref| >= 2%s); worst excess %.3e" % (
+        what, err.max(), O_TOL, "; 2^-7 sum p|V| where larger" if A_ref is not None else "", (err - tol).max())
+    if (err > O_TOL).any() and os.environ.get("CSV_TOL_LOG"):   # which cases needed more than the plain 1e-2 (listed in S20)
         with open(os.environ["CSV_TOL_LOG"], "a") as f:
             f.write("%s: max err %.4e at |O_ref| %.3f\n" % (what, err.max(), float(mag.reshape(-1)[err.argmax()])))
     lerr = np.abs(LSE - LSE_ref).max()

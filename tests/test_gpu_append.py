@@ -8,7 +8,8 @@ import torch
 
 from paper_2606_01839_b200 import binding as B
 from paper_2606_01839_b200 import synth
-from harness import Scenario, assert_close, bf16_dev_to_f64, dev, oracle_attention, run_attention, u16_dev
+from harness import (Scenario, assert_close, bf16_dev_to_f64, dev, oracle_abs_weighted, oracle_attention, run_attention,
+                     u16_dev)
 
 pytestmark = pytest.mark.gpu
 
@@ -22,7 +23,8 @@ def step_case(oracle, seed, Hq, Hkv, d, convs, mpt=0, poison=False, v_mean=0.0, 
     q = synth.normal_bf16(rng, (sum(q_lens), Hq, d), std=qscale)
     O, LSE, info = run_attention(sc, q_lens, q, mpt=mpt, which="both")
     O_ref, LSE_ref = oracle_attention(sc, q_lens, q)
-    return assert_close(O, LSE, O_ref, LSE_ref, what or "step"), info
+    A_ref = oracle_abs_weighted(sc, q_lens, q) if qscale > 1.0 else None   # peaked softmax: DESIGN.md S20
+    return assert_close(O, LSE, O_ref, LSE_ref, what or "step", A_ref=A_ref), info
 
 
 @pytest.mark.parametrize("Hq,Hkv,d", [(32, 8, 128), (64, 8, 128), (4, 1, 64), (8, 8, 64), (16, 2, 128), (8, 8, 128), (8, 4, 128),

@@ -9,7 +9,7 @@ import torch
 
 from paper_2606_01839_b200 import binding as B
 from paper_2606_01839_b200 import synth
-from harness import Scenario, assert_close, oracle_attention, run_attention
+from harness import Scenario, assert_close, oracle_abs_weighted, oracle_attention, run_attention
 
 pytestmark = pytest.mark.gpu
 
@@ -21,7 +21,8 @@ def decode_case(oracle, seed, Hq, Hkv, d, kv_lens, mpt=0, poison=False, v_mean=0
     q = synth.normal_bf16(rng, (len(kv_lens), Hq, d), std=qscale)
     O, LSE, info = run_attention(sc, q_lens, q, mpt=mpt, which="decode")
     O_ref, LSE_ref = oracle_attention(sc, q_lens, q)
-    return assert_close(O, LSE, O_ref, LSE_ref, what or "decode"), info, (O, LSE)
+    A_ref = oracle_abs_weighted(sc, q_lens, q) if qscale > 1.0 else None   # peaked softmax: DESIGN.md S20
+    return assert_close(O, LSE, O_ref, LSE_ref, what or "decode", A_ref=A_ref), info, (O, LSE)
 
 
 def test_config1_tiny_decode(oracle):

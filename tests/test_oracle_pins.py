@@ -170,6 +170,23 @@ def test_empty_cache(oracle):
     assert O.shape == (0, 4, 16) and LSE.shape == (0, 4)
 
 
+def test_decode_row_on_an_empty_cache_is_zero_and_minus_infinity(oracle):
+    # SURVEY 8c O1 step 6 / conserve_kv.h a4: a decode row with no key to attend to gives O = 0, LSE = -inf.  It is
+    # also the limit of the merge identity: merging it with any other part leaves that part unchanged.
+    q = synth.normal_bf16(np.random.default_rng(3), (1, 4, 16))
+    K = np.zeros((0, 2, 16), dtype=np.uint16)
+    O, LSE = oracle.attention(q, K, K)
+    assert O.shape == (1, 4, 16) and np.all(O == 0.0) and np.all(np.isneginf(LSE))
+    Kb = synth.normal_bf16(np.random.default_rng(4), (5, 2, 16))
+    Vb = synth.normal_bf16(np.random.default_rng(5), (5, 2, 16))
+    Ob, Lb = oracle.attention(q, Kb[:1], Vb[:1])     # R = 1, L = 1 is the smallest ordinary case
+    for h in range(4):
+        Om, Lm = oracle.merge(O[0, h], LSE[0, h], Ob[0, h], Lb[0, h])
+        assert np.allclose(Om, Ob[0, h], atol=1e-15) and abs(Lm - Lb[0, h]) <= 1e-15
+    with pytest.raises(ValueError):                  # R > L stays an error everywhere else
+        oracle.attention(np.zeros((2, 4, 16), dtype=np.uint16), Kb[:1], Vb[:1])
+
+
 # ------------------------------------------------------------------ O1 whole
 
 def test_brute_force_tiny(oracle):
