@@ -246,11 +246,18 @@ int kv_handoff_direct_batch(kv_pool_t* dst, int32_t n, const void* const* h_d_k,
  *   Opens of the same allocation are counted (several exported pointers may
  *   share one allocation); the mapping goes away with the last close.
  * csv_ipc_close: d_ptr is what csv_ipc_open returned (one close per open).
+ * csv_ipc_copy: copy-engine transfer (cudaMemcpyAsync, device to device) of
+ *   `bytes` bytes between two device pointers of which either may be a
+ *   csv_ipc_open mapping: the staged route's "send the message" step
+ *   (kv_pack locally, copy the staging message to the decoder, kv_unpack there),
+ *   kept as the comparison arm of kv_handoff_direct.  Enqueued
+ *   on `stream`, never synchronises.
  * Errors: CSV_E_INVAL bad argument / unknown pointer, CSV_E_CUDA otherwise. */
 #define CSV_IPC_HANDLE_BYTES 64
 int csv_ipc_export(const void* d_ptr, void* out_handle, uint64_t* out_offset);
 int csv_ipc_open(const void* handle, uint64_t offset, void** out_d_ptr);
 int csv_ipc_close(void* d_ptr);
+int csv_ipc_copy(void* d_dst, const void* d_src, size_t bytes, void* stream);
 
 /* Tail-step KV append ("appending one new entry"; PAPER.md:94
  * "only calculating new KV cache entries for the appended tokens"): writes the
@@ -386,18 +393,28 @@ int csv_tail_step(const csv_plan_t* plan, kv_pool_t* pool, int32_t layer, const 
 
 /* ------------------------------------------------------------------------
  * End-to-end convenience with HOST buffers (what bench.py's "e2e" times): one
- * decode tail step of one layer.  Plans from the host lengths, copies
- * h_q, h_k_new, h_v_new ([batch][Hq|Hkv][d] bf16, one new token per
- * conversation, already counted in h_kv_lens) and h_block_tables to the
- * device workspace, runs paged_decode_step (= kv_append_tokens + paged_decode_attn), copies O and
- * LSE back to h_out / h_lse and synchronises `stream`.
- * d_workspace: >= csv_tail_step_host_workspace_bytes(...), 128-byte aligned.
+ * tail step (decode rows and appended chunks in one iteration)
+ * over layers [layer_begin, layer_begin + n_layers) of the pool.
+ * h_q_lens[batch]: 1 = decode row, > 1 = appended chunk, 0 = inert; NULL = all 1.
+ * h_kv_lens[batch]: cached tokens INCLUDING the new rows.  Per layer the rows
+ * are ordered as in a plan (total_q = sum of q_lens):
+ *   h_q, h_out:         [n_layers][total_q][Hq][d]  bf16
+ *   h_k_new, h_v_new:   [n_layers][total_q][Hkv][d] bf16
+ *   h_lse:              [n_layers][total_q][Hq]     fp32
+ *   h_block_tables:     [batch][max_blocks] (one table serves all layers)
+ * The call enqueues the host->device copies, builds ONE plan for the step while
+ * they fly (lengths are per step, not per layer), runs csv_tail_step on every
+ * layer, copies O and LSE back and synchronises `stream`.  Host buffers should
+ * be pinned.  d_workspace: >= csv_tail_step_host_workspace_bytes(...), 128-byte
+ * aligned.  Errors as csv_plan_create / csv_tail_step; nothing is launched on
+ * CSV_E_INVAL / CSV_E_NOMEM.
  * ---------------------------------------------------------------------- */
-size_t csv_tail_step_host_workspace_bytes(const csv_attn_shape* shape, const int32_t* h_kv_lens,
-                                          int32_t batch, int32_t max_blocks, int32_t max_partition_tokens);
-int csv_tail_step_host(kv_pool_t* pool, int32_t layer, const csv_attn_shape* shape, int32_t batch,
-                       const int32_t* h_kv_lens, const void* h_q, const void* h_k_new, const void* h_v_new,
-                       const int32_t* h_block_tables, int32_t max_blocks, int32_t max_partition_tokens,
+size_t csv_tail_step_host_workspace_bytes(const csv_attn_shape* shape, const int32_t* h_q_lens, const int32_t* h_kv_lens,
+                                          int32_t batch, int32_t max_blocks, int32_t n_layers,
+                                          int32_t max_partition_tokens);
+int csv_tail_step_host(kv_pool_t* pool, int32_t layer_begin, int32_t n_layers, const csv_attn_shape* shape, int32_t batch,
+                       const int32_t* h_q_lens, const int32_t* h_kv_lens, const void* h_q, const void* h_k_new,
+                       const void* h_v_new, const int32_t* h_block_tables, int32_t max_blocks, int32_t max_partition_tokens,
                        void* d_workspace, size_t ws_bytes, void* h_out, float* h_lse, void* stream);
 
 #ifdef __cplusplus

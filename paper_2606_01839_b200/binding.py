@@ -23,7 +23,7 @@ SYMBOLS = [
     "kv_unpack", "kv_pack_batch", "kv_unpack_batch", "kv_append_tokens", "csv_plan_workspace_bytes",
     "csv_plan_create", "csv_plan_destroy", "csv_plan_info", "csv_plan_total_q", "csv_plan_decode_items",
     "csv_plan_append_items", "paged_decode_attn", "paged_decode_step", "append_prefill_attn", "csv_tail_step_host_workspace_bytes",
-    "csv_tail_step_host", "kv_handoff_direct", "kv_handoff_direct_batch", "csv_ipc_export", "csv_ipc_open", "csv_ipc_close", "csv_tail_step",
+    "csv_tail_step_host", "kv_handoff_direct", "kv_handoff_direct_batch", "csv_ipc_export", "csv_ipc_open", "csv_ipc_close", "csv_ipc_copy", "csv_tail_step",
 ]
 IPC_HANDLE_BYTES = 64
 
@@ -85,6 +85,7 @@ def lib():
             "csv_ipc_export": (ctypes.c_int, [vp, vp, ctypes.POINTER(ctypes.c_uint64)]),
             "csv_ipc_open": (ctypes.c_int, [vp, ctypes.c_uint64, pvp]),
             "csv_ipc_close": (ctypes.c_int, [vp]),
+            "csv_ipc_copy": (ctypes.c_int, [vp, vp, sz, vp]),
             "csv_plan_workspace_bytes": (sz, [pshape, pi32, pi32, i32, i32]),
             "csv_plan_create": (ctypes.c_int, [pshape, pi32, pi32, i32, i32, vp, sz, vp, pvp]),
             "csv_plan_destroy": (ctypes.c_int, [vp]),
@@ -96,9 +97,9 @@ def lib():
             "append_prefill_attn": (ctypes.c_int, [vp, vp, i32, vp, vp, i32, vp, vp, vp]),
             "paged_decode_step": (ctypes.c_int, [vp, vp, i32, vp, vp, vp, vp, i32, vp, vp, vp]),
             "csv_tail_step": (ctypes.c_int, [vp, vp, i32, vp, vp, vp, vp, i32, vp, vp, vp]),
-            "csv_tail_step_host_workspace_bytes": (sz, [pshape, pi32, i32, i32, i32]),
-            "csv_tail_step_host": (ctypes.c_int, [vp, i32, pshape, i32, pi32, vp, vp, vp, pi32, i32, i32, vp, sz, vp,
-                                                  vp, vp]),
+            "csv_tail_step_host_workspace_bytes": (sz, [pshape, pi32, pi32, i32, i32, i32, i32]),
+            "csv_tail_step_host": (ctypes.c_int, [vp, i32, i32, pshape, i32, pi32, pi32, vp, vp, vp, pi32, i32, i32, vp, sz,
+                                                  vp, vp, vp]),
         }
         for name, (res, args) in sig.items():
             fn = getattr(L, name)
@@ -300,6 +301,11 @@ def csv_ipc_close(ptr):
     _check("csv_ipc_close", lib().csv_ipc_close(ctypes.c_void_p(ptr)))
 
 
+def csv_ipc_copy(dst, src, nbytes, stream=None):
+    """Copy-engine transfer between device buffers (torch tensors or raw pointers, e.g. a csv_ipc_open mapping)."""
+    _check("csv_ipc_copy", lib().csv_ipc_copy(_ptr(dst), _ptr(src), int(nbytes), _stream(stream)))
+
+
 def csv_plan_workspace_bytes(shape, q_lens, kv_lens, max_partition_tokens=0):
     q, pq = _i32(q_lens)
     _, pk = _i32(kv_lens)
@@ -390,17 +396,20 @@ def kv_append_tokens(pool, plan, d_k_new, d_v_new, d_block_tables, max_blocks, s
                                                       _ptr(d_block_tables), max_blocks, _stream(stream)))
 
 
-def csv_tail_step_host_workspace_bytes(shape, kv_lens, max_blocks, max_partition_tokens=0):
+def csv_tail_step_host_workspace_bytes(shape, kv_lens, max_blocks, max_partition_tokens=0, q_lens=None, n_layers=1):
     k, pk = _i32(kv_lens)
-    return int(lib().csv_tail_step_host_workspace_bytes(ctypes.byref(shape), pk, len(k), max_blocks,
+    pq = _i32(q_lens)[1] if q_lens is not None else None
+    return int(lib().csv_tail_step_host_workspace_bytes(ctypes.byref(shape), pq, pk, len(k), max_blocks, n_layers,
                                                         max_partition_tokens))
 
 
 def csv_tail_step_host(pool, layer, shape, kv_lens, h_q, h_k_new, h_v_new, h_block_tables, max_blocks, workspace, h_out,
-                       h_lse, max_partition_tokens=0, stream=None):
-    """One decode tail step with HOST (pinned torch) buffers; synchronises the stream before returning."""
+                       h_lse, max_partition_tokens=0, stream=None, q_lens=None, n_layers=1):
+    """One tail step (decode rows + appended chunks, layers [layer, layer + n_layers)) with HOST (pinned torch) buffers;
+    synchronises the stream before returning."""
     k, pk = _i32(kv_lens)
+    q = _i32(q_lens) if q_lens is not None else None
     _check("csv_tail_step_host", lib().csv_tail_step_host(
-        pool.handle, layer, ctypes.byref(shape), len(k), pk, _ptr(h_q), _ptr(h_k_new), _ptr(h_v_new),
-        ctypes.cast(_ptr(h_block_tables), ctypes.POINTER(ctypes.c_int32)), max_blocks, max_partition_tokens,
+        pool.handle, layer, n_layers, ctypes.byref(shape), len(k), q[1] if q else None, pk, _ptr(h_q), _ptr(h_k_new),
+        _ptr(h_v_new), ctypes.cast(_ptr(h_block_tables), ctypes.POINTER(ctypes.c_int32)), max_blocks, max_partition_tokens,
         _ptr(workspace), workspace.numel() * workspace.element_size(), _ptr(h_out), _ptr(h_lse), _stream(stream)))

@@ -202,6 +202,13 @@ int csv_ipc_close(void* d_ptr) {
     return CSV_E_INVAL;
 }
 
+int csv_ipc_copy(void* d_dst, const void* d_src, size_t bytes, void* stream) {
+    if (!d_dst || !d_src) return CSV_E_INVAL;
+    if (bytes == 0) return CSV_OK;
+    CSV_CUDA_TRY(cudaMemcpyAsync(d_dst, d_src, bytes, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+    return CSV_OK;
+}
+
 // Points a host-built plan at its device workspace and enqueues the upload of its work lists.
 static int plan_attach(csv_plan* p, void* d_workspace, size_t ws_bytes, void* stream) {
     if (!aligned(d_workspace, 128)) return CSV_E_INVAL;
@@ -313,7 +320,7 @@ int csv_tail_step(const csv_plan_t* plan, kv_pool_t* pool, int32_t layer, const 
 struct TailLayout {
     size_t plan, q, k, v, tables, out, lse, total;
 };
-static TailLayout tail_layout(const csv_attn_shape* s, int batch, int max_blocks, size_t plan_bytes) {
+static TailLayout tail_layout(const csv_attn_shape* s, int64_t rows, int batch, int max_blocks, size_t plan_bytes) {
     TailLayout L;
     size_t off = 0;
     auto take = [&](size_t b) {
@@ -321,68 +328,81 @@ static TailLayout tail_layout(const csv_attn_shape* s, int batch, int max_blocks
         off = (off + b + 127) / 128 * 128;
         return at;
     };
-    L.q = take((size_t)batch * s->num_q_heads * s->head_dim * 2);
-    L.k = take((size_t)batch * s->num_kv_heads * s->head_dim * 2);
-    L.v = take((size_t)batch * s->num_kv_heads * s->head_dim * 2);
+    L.q = take((size_t)rows * s->num_q_heads * s->head_dim * 2);
+    L.k = take((size_t)rows * s->num_kv_heads * s->head_dim * 2);
+    L.v = take((size_t)rows * s->num_kv_heads * s->head_dim * 2);
     L.tables = take((size_t)batch * max_blocks * 4);
-    L.out = take((size_t)batch * s->num_q_heads * s->head_dim * 2);
-    L.lse = take((size_t)batch * s->num_q_heads * 4);
+    L.out = take((size_t)rows * s->num_q_heads * s->head_dim * 2);
+    L.lse = take((size_t)rows * s->num_q_heads * 4);
     L.plan = take(plan_bytes);   // last: its size is only known once the plan is built
     L.total = off;
     return L;
 }
 
-size_t csv_tail_step_host_workspace_bytes(const csv_attn_shape* shape, const int32_t* h_kv_lens, int32_t batch,
-                                          int32_t max_blocks, int32_t max_partition_tokens) {
-    if (!shape || batch <= 0 || max_blocks <= 0 || !h_kv_lens) return 0;
-    std::vector<int32_t> ones((size_t)batch, 1);
-    const size_t pb = csv_plan_workspace_bytes(shape, ones.data(), h_kv_lens, batch, max_partition_tokens);
-    if (pb == 0) return 0;
-    return tail_layout(shape, batch, max_blocks, pb).total;
+static int64_t host_step_rows(const int32_t* h_q_lens, int32_t batch) {   // total_q of one layer; -1 = bad lengths
+    if (!h_q_lens) return batch;
+    int64_t t = 0;
+    for (int b = 0; b < batch; ++b) {
+        if (h_q_lens[b] < 0) return -1;
+        t += h_q_lens[b];
+    }
+    return t;
 }
 
-int csv_tail_step_host(kv_pool_t* pool, int32_t layer, const csv_attn_shape* shape, int32_t batch,
-                       const int32_t* h_kv_lens, const void* h_q, const void* h_k_new, const void* h_v_new,
-                       const int32_t* h_block_tables, int32_t max_blocks, int32_t max_partition_tokens, void* d_workspace,
-                       size_t ws_bytes, void* h_out, float* h_lse, void* stream) {
-    if (!pool || !shape || batch <= 0 || !h_kv_lens || !h_q || !h_k_new || !h_v_new || !h_block_tables || !h_out ||
-        !h_lse || !d_workspace || !aligned(d_workspace, 128) || max_blocks <= 0)
+size_t csv_tail_step_host_workspace_bytes(const csv_attn_shape* shape, const int32_t* h_q_lens, const int32_t* h_kv_lens,
+                                          int32_t batch, int32_t max_blocks, int32_t n_layers, int32_t max_partition_tokens) {
+    if (!shape || batch <= 0 || max_blocks <= 0 || n_layers <= 0 || !h_kv_lens) return 0;
+    const int64_t rows = host_step_rows(h_q_lens, batch);
+    if (rows <= 0) return 0;
+    std::vector<int32_t> ones;
+    if (!h_q_lens) ones.assign((size_t)batch, 1);
+    const size_t pb = csv_plan_workspace_bytes(shape, h_q_lens ? h_q_lens : ones.data(), h_kv_lens, batch, max_partition_tokens);
+    if (pb == 0) return 0;
+    return tail_layout(shape, rows * n_layers, batch, max_blocks, pb).total;
+}
+
+int csv_tail_step_host(kv_pool_t* pool, int32_t layer_begin, int32_t n_layers, const csv_attn_shape* shape, int32_t batch,
+                       const int32_t* h_q_lens, const int32_t* h_kv_lens, const void* h_q, const void* h_k_new,
+                       const void* h_v_new, const int32_t* h_block_tables, int32_t max_blocks, int32_t max_partition_tokens,
+                       void* d_workspace, size_t ws_bytes, void* h_out, float* h_lse, void* stream) {
+    if (!pool || !shape || batch <= 0 || n_layers <= 0 || !h_kv_lens || !h_q || !h_k_new || !h_v_new || !h_block_tables ||
+        !h_out || !h_lse || !d_workspace || !aligned(d_workspace, 128) || max_blocks <= 0)
         return CSV_E_INVAL;
-    if (layer < 0 || layer >= pool->desc.num_layers || !same_shape(pool->desc, *shape)) return CSV_E_INVAL;
+    if (layer_begin < 0 || layer_begin + (int64_t)n_layers > pool->desc.num_layers || !same_shape(pool->desc, *shape))
+        return CSV_E_INVAL;
     if (shape->num_q_heads <= 0 || shape->num_q_heads % shape->num_kv_heads != 0) return CSV_E_INVAL;
+    const int64_t rows = host_step_rows(h_q_lens, batch);   // per layer
+    if (rows <= 0 || rows * n_layers > INT32_MAX) return CSV_E_INVAL;
     // The plan's size is not known before it is built, so the fixed-size buffers sit in front of it: their copies
     // are enqueued first and fly while the host plans.
-    const size_t qb = (size_t)batch * shape->num_q_heads * shape->head_dim * 2;
-    const size_t kb = (size_t)batch * shape->num_kv_heads * shape->head_dim * 2;
-    const TailLayout L = tail_layout(shape, batch, max_blocks, 0);   // L.plan is the END region here (see tail_layout)
+    const size_t q_layer = (size_t)rows * shape->num_q_heads * shape->head_dim * 2;
+    const size_t k_layer = (size_t)rows * shape->num_kv_heads * shape->head_dim * 2;
+    const size_t lse_layer = (size_t)rows * shape->num_q_heads * 4;
+    const TailLayout L = tail_layout(shape, rows * n_layers, batch, max_blocks, 0);   // L.plan is the END region here
     if (ws_bytes < L.total) return CSV_E_NOMEM;
     uint8_t* ws = (uint8_t*)d_workspace;
     cudaStream_t st = (cudaStream_t)stream;
     cudaError_t e;
-    if ((e = cudaMemcpyAsync(ws + L.q, h_q, qb, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
-        (e = cudaMemcpyAsync(ws + L.k, h_k_new, kb, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
-        (e = cudaMemcpyAsync(ws + L.v, h_v_new, kb, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
+    if ((e = cudaMemcpyAsync(ws + L.q, h_q, q_layer * n_layers, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(ws + L.k, h_k_new, k_layer * n_layers, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(ws + L.v, h_v_new, k_layer * n_layers, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
         (e = cudaMemcpyAsync(ws + L.tables, h_block_tables, (size_t)batch * max_blocks * 4, cudaMemcpyHostToDevice, st)) !=
             cudaSuccess)
         return csv_set_cuda_error((int)e);
-    std::vector<int32_t> ones((size_t)batch, 1);
+    std::vector<int32_t> ones;
+    if (!h_q_lens) ones.assign((size_t)batch, 1);
     int err;
-    csv_plan_t* plan = csv_plan_build_host(shape, ones.data(), h_kv_lens, batch, max_partition_tokens, &err);   // planned once
+    csv_plan_t* plan =   // one plan serves every layer of the step (lengths are per step, not per layer)
+        csv_plan_build_host(shape, h_q_lens ? h_q_lens : ones.data(), h_kv_lens, batch, max_partition_tokens, &err);
     if (!plan) return err;
     int rc = ws_bytes - L.plan < plan->lay.total ? CSV_E_NOMEM : plan_attach(plan, ws + L.plan, ws_bytes - L.plan, stream);
-    if (rc != CSV_OK) {
-        csv_plan_destroy(plan);
-        return rc;
-    }
-    // the new token's K/V go to `layer` of the pool: view that layer as a 1-layer pool
-    kv_pool layer_view = layer_view_of(pool, layer);
-    if (rc == CSV_OK)   // new-token KV write fused into the decode launch
-        rc = paged_decode_step(plan, &layer_view, 0, ws + L.q, ws + L.k, ws + L.v, (const int32_t*)(ws + L.tables), max_blocks,
-                               ws + L.out, (float*)(ws + L.lse), stream);
+    for (int l = 0; rc == CSV_OK && l < n_layers; ++l)   // KV write of every new row + decode rows + appended chunks
+        rc = csv_tail_step(plan, pool, layer_begin + l, ws + L.q + l * q_layer, ws + L.k + l * k_layer, ws + L.v + l * k_layer,
+                           (const int32_t*)(ws + L.tables), max_blocks, ws + L.out + l * q_layer,
+                           (float*)(ws + L.lse + l * lse_layer), stream);
     if (rc == CSV_OK) {
-        if ((e = cudaMemcpyAsync(h_out, ws + L.out, qb, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
-            (e = cudaMemcpyAsync(h_lse, ws + L.lse, (size_t)batch * shape->num_q_heads * 4, cudaMemcpyDeviceToHost, st)) !=
-                cudaSuccess ||
+        if ((e = cudaMemcpyAsync(h_out, ws + L.out, q_layer * n_layers, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
+            (e = cudaMemcpyAsync(h_lse, ws + L.lse, lse_layer * n_layers, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
             (e = cudaStreamSynchronize(st)) != cudaSuccess)
             rc = csv_set_cuda_error((int)e);
     }

@@ -419,7 +419,9 @@ int launch_append_attn_tc2(const csv_plan* plan, const kv_pool* pool, int layer,
     if (e3 && atoi(e3) == 3) {
         static PerDeviceOnce attr3;
         CSV_CUDA_TRY(once_per_device(attr3, [] {
-            return cudaFuncSetAttribute(append_tc2_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes2(3));
+            cudaError_t e = cudaFuncSetAttribute(append_tc2_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes2(3));
+            if (e == cudaSuccess) e = cudaFuncSetAttribute(append_tc2_kernel<3>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+            return e;
         }));
         append_tc2_kernel<3><<<grid, kT2Threads, smem_bytes2(3), (cudaStream_t)stream>>>(p);
     } else {

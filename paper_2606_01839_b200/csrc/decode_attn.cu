@@ -25,6 +25,8 @@
 #include <math.h>
 #include <stdlib.h>
 
+#include <algorithm>
+
 #include "common.cuh"
 #include "internal.h"
 
@@ -45,6 +47,7 @@ struct DecodeParams {
     uint8_t* pool_layer_w;  // same address as pool_layer, writable (fused step)
     int32_t max_blocks, Hq, Hkv, G;
     float scale_log2;
+    int32_t l2_prefetch;   // blocks ahead of the ring that lane 0 asks the L2 to fetch (0 = off)
 };
 
 // One warp per (merge group, query head of the group): log-sum-exp merge of the group's partials in
@@ -265,6 +268,19 @@ __global__ void __launch_bounds__(WARPS * 32, WARPS == 8 ? 1 : 512 / (WARPS * 32
                     bulk_g2s(dst + TB, src + kv_stride, TB, &bars[stage]);
                 }
             }
+            if (p.l2_prefetch > 0) {
+                // the shared-memory ring covers the L2 -> SM latency only; the HBM -> L2 leg is started l2_prefetch blocks early
+                const int far = nxt + p.l2_prefetch;
+                if (far < nblk && (far >> 5) <= grp_cur + 1) {
+                    const int id = (far >> 5) == grp_cur ? __shfl_sync(0xffffffffu, ids_cur, far & 31)
+                                                         : __shfl_sync(0xffffffffu, ids_nxt, far & 31);
+                    if (lane == 0) {
+                        const uint8_t* src = head_base + (size_t)id * blk_stride;
+                        l2_prefetch(src, TB);
+                        l2_prefetch(src + kv_stride, TB);
+                    }
+                }
+            }
             if (i == pf_at && has_next) {
                 const int nn = n0.w - n0.z;
                 ids_pref = lane < nn ? __ldg(p.tables + (size_t)n0.x * p.max_blocks + n0.z + lane) : 0;
@@ -308,7 +324,11 @@ int launch_decode_t(const csv_plan* plan, const DecodeParams& p, cudaStream_t st
     const size_t smem = (size_t)WARPS * STAGES * 2 * TB + (size_t)WARPS * STAGES * 8;
     static PerDeviceOnce attr;
     CSV_CUDA_TRY(once_per_device(attr, [&] {
-        return cudaFuncSetAttribute(decode_kernel<D, STAGES, WARPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t e = cudaFuncSetAttribute(decode_kernel<D, STAGES, WARPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        // the slim variant runs BESIDE the append CTA: the SM must be carved for both kernels' shared memory at once
+        if (e == cudaSuccess && WARPS != 8)
+            e = cudaFuncSetAttribute(decode_kernel<D, STAGES, WARPS>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+        return e;
     }));
     CSV_CUDA_TRY(launch_pdl(decode_kernel<D, STAGES, WARPS>, dim3(plan->decode_grid), dim3(WARPS * 32), smem, stream, p));
     const int ng = (int)plan->decode_groups.size();
@@ -349,6 +369,8 @@ int launch_decode(const csv_plan* plan, const kv_pool* pool, int layer, const vo
     p.Hkv = plan->shape.num_kv_heads;
     p.G = p.Hq / p.Hkv;
     p.scale_log2 = (float)(1.4426950408889634 / sqrt((double)s.head_dim));
+    p.l2_prefetch = 0;
+    if (const char* e = getenv("CSV_X_DECODE_PF")) p.l2_prefetch = std::max(0, std::min(24, atoi(e)));   // experiment knob
     if (s.head_dim == 128) {
         if (plan->decode_warps == 2) return launch_decode_t<128, 4, 2>(plan, p, (cudaStream_t)stream);
         return launch_decode_t<128, 3, 8>(plan, p, (cudaStream_t)stream);

@@ -49,7 +49,9 @@ static void plan_decode(csv_plan* p) {
     // CTAs: one per SM, fewer when there is under 4 blocks of work per warp
     const int WPC = p->decode_warps;   // warp-workers per CTA
     int64_t want = (units + (int64_t)WPC * 4 - 1) / ((int64_t)WPC * 4);
-    p->decode_grid = (int)std::max<int64_t>(1, std::min<int64_t>(p->num_sms, want));
+    int64_t max_grid = p->num_sms;
+    if (const char* e = getenv("CSV_X_DECODE_MULT")) max_grid *= std::max(1, atoi(e));   // experiment knob: slim CTAs per SM
+    p->decode_grid = (int)std::max<int64_t>(1, std::min<int64_t>(max_grid, want));
     if (const char* e = getenv("CSV_X_DECODE_GRID")) p->decode_grid = std::max(1, std::min(p->decode_grid, atoi(e)));   // experiment knob
     const int64_t W = (int64_t)p->decode_grid * WPC;
     p->worker_begin.assign((size_t)W + 1, 0);

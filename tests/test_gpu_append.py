@@ -183,6 +183,52 @@ def test_tail_step_mixed_batch_one_call(oracle):
         B.csv_tail_step(plan, sc.pool, layer, u16_dev(q), None, u16_dev(v_new), sc.d_tables, sc.max_blocks, d_out, d_lse)
 
 
+def test_tail_step_host_mixed_batch_two_layers(oracle):
+    """csv_tail_step_host with q_lens and n_layers = 2: one plan, one table upload, both layers' new rows written, decode
+    rows and appended chunks attended on each layer; host results against the oracle, whole pool against its scatter."""
+    from harness import dev_to_u16
+    rng = np.random.default_rng(93)
+    Hq, Hkv, d, NL = 32, 8, 128, 2
+    kv_lens = [700, 33, 2049, 300, 16, 1, 129]
+    q_lens = [1, 32, 1, 257, 1, 1, 0]
+    sc = Scenario(oracle, rng, Hq, Hkv, d, kv_lens, NL=NL, poison=True)
+    full = sc.image.copy()
+    for b, (t, m) in enumerate(zip(kv_lens, q_lens)):
+        full = oracle.scatter(full, NL, sc.num_blocks, Hkv, d, sc.K[b], sc.V[b], t, 0, sc.tables[b])
+        if t - m > 0:   # the cache before the step: both layers without the step's own rows
+            sc.image = oracle.scatter(sc.image, NL, sc.num_blocks, Hkv, d, sc.K[b][:, :t - m], sc.V[b][:, :t - m], t - m, 0,
+                                      sc.tables[b])
+    sc.upload()
+    rows = [(b, t, m) for b, (t, m) in enumerate(zip(kv_lens, q_lens)) if m > 0]
+    k_new = np.stack([np.concatenate([sc.K[b][l, t - m:t] for b, t, m in rows]) for l in range(NL)])
+    v_new = np.stack([np.concatenate([sc.V[b][l, t - m:t] for b, t, m in rows]) for l in range(NL)])
+    total_q = sum(q_lens)
+    q = synth.normal_bf16(rng, (NL, total_q, Hq, d))
+    shape = B.attn_shape(Hq, Hkv, d)
+    tabs = np.where(sc.h_tables < 0, 0, sc.h_tables).astype(np.int32)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    h_out = torch.full((NL, total_q, Hq, d), 0x7FC0, dtype=torch.int16).pin_memory()
+    h_lse = torch.full((NL, total_q, Hq), float("nan"), dtype=torch.float32).pin_memory()
+    nbytes = B.csv_tail_step_host_workspace_bytes(shape, kv_lens, sc.max_blocks, q_lens=q_lens, n_layers=NL)
+    ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    B.csv_tail_step_host(sc.pool, 0, shape, kv_lens, pin(q.view(np.int16)), pin(k_new.view(np.int16)), pin(v_new.view(np.int16)),
+                         pin(tabs), sc.max_blocks, ws, h_out, h_lse, q_lens=q_lens, n_layers=NL)
+    got = dev_to_u16(sc.d_image)
+    assert np.array_equal(got, full), "pool after csv_tail_step_host differs from the oracle's scatter"
+    for l in range(NL):
+        O = synth.bf16_bits_to_f32(h_out[l].numpy().view(np.uint16)).astype(np.float64)
+        O_ref, LSE_ref = oracle_attention(sc, q_lens, q[l], layer=l)
+        assert_close(O, h_lse[l].numpy().astype(np.float64), O_ref, LSE_ref, what="host step layer %d" % l)
+    with pytest.raises(B.CsvError):   # layers past the pool, and a workspace sized for one layer only
+        B.csv_tail_step_host(sc.pool, 1, shape, kv_lens, pin(q.view(np.int16)), pin(k_new.view(np.int16)),
+                             pin(v_new.view(np.int16)), pin(tabs), sc.max_blocks, ws, h_out, h_lse, q_lens=q_lens, n_layers=NL)
+    small = torch.empty(B.csv_tail_step_host_workspace_bytes(shape, kv_lens, sc.max_blocks, q_lens=q_lens, n_layers=1),
+                        dtype=torch.uint8, device="cuda")
+    with pytest.raises(B.CsvError):
+        B.csv_tail_step_host(sc.pool, 0, shape, kv_lens, pin(q.view(np.int16)), pin(k_new.view(np.int16)),
+                             pin(v_new.view(np.int16)), pin(tabs), sc.max_blocks, small, h_out, h_lse, q_lens=q_lens, n_layers=NL)
+
+
 def test_append_spike_sweep_sees_every_block(oracle):
     """SURVEY §8c item 1 for the tcgen05 kernel: one key carries ~all the weight for every row that may see it and its V
     is a +-1 pattern; the spike sits on the first / last block of each KV partition, around the prefix / chunk boundary

@@ -268,4 +268,5 @@ def test_handoff_across_two_ranks_direct_and_staged():
     assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-2000:]
     line = [ln for ln in r.stdout.splitlines() if ln.startswith("{")][-1]
     out = json.loads(line)
-    assert out["bit_exact_direct"] and out["bit_exact_staged"] and out["convs"] == 5
+    assert out["bit_exact_direct"] and out["bit_exact_staged"] and out["bit_exact_copy"] and out["convs"] == 5
+    assert out["memcpy_peer_gbs"] > 0 and out["copy_payload_gbs"] > 0          # the cudaMemcpyAsync comparison arm ran

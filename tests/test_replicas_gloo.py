@@ -113,3 +113,22 @@ def test_handoff_tickets_travel_from_decoder_to_prefiller():
         assert False
     except ValueError:
         pass
+
+
+def test_bench_launches_its_own_ranks_when_torchrun_did_not():
+    # `python bench.py --gpus 2` with no WORLD_SIZE in the environment must become two ranks on its own (a plain
+    # --gpus N run measured one replica).  The reference arm runs without a GPU: rank 0 times the oracle, rank 1 exits 0.
+    import json
+    import subprocess
+    import sys
+
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--impl", "reference", "--gpus", "2", "--steps", "1",
+                        "--warmup", "0"], cwd=root, env=env, capture_output=True, text=True, timeout=900)
+    assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-2000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1, lines                      # rank 0 alone prints
+    out = json.loads(lines[0])
+    assert out["impl"] == "reference" and out["n_gpus"] == 2 and out["value"] > 0
+    assert out["cpu_baseline"]["kind"] == "oracle" and out["e2e"]["h2d_bytes_per_step"] == 0
