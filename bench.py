@@ -390,19 +390,37 @@ def leg_long_context_extras(wl, L, pk, iters=6):
     blocks = [roofline_block("append_tc2_kernel", "configs[4]", "tensor", app.append_flops(), ap, pk,
                              note="per append_prefill_attn call on one layer: 4 chunks x 256 tokens, prefix 130816")]
 
-    def mixed():
+    def parts():
         for layer in range(L):
             wl.decode(layer=layer)
             app.append(layer=layer)
 
-    g = graph_of(mixed)
-    mx = time_calls(g.replay if g else mixed, 3, 1)
+    g = graph_of(parts)
+    mx = time_calls(g.replay if g else parts, 3, 1)
     dec = time_calls(lambda: [wl.decode(layer=l) for l in range(L)], 3, 1)
-    step = {"config": "configs[4]", "what": "decode of all 16 conversations + the 4 appended chunks on each of %d layers "
-            "(paged_decode_attn + append_prefill_attn per layer), CUDA-graph replay" % L,
-            "ms_median": mx["median_ms"], "ms_min": mx["min_ms"], "decode_only_ms": dec["median_ms"],
-            "append_only_ms_per_layer": ap["median_ms"], "sum_of_parts_ms": dec["median_ms"] + L * ap["median_ms"],
-            "append_tflops_inside_step_vs_sustained_peak": None}
+    # the same step in ONE call per layer (csv_tail_step, attention only: S14's rows are in the pool): decode rows and
+    # chunks as work items of one persistent launch (tail_fused.cu).  The 4 chunks are extra batch entries whose tables
+    # name the blocks of conversations 0-3.
+    from paper_2606_01839_b200 import synth
+    Lc = synth.config_lengths(5)
+    mixed = wl.with_extra_chunks(Lc["append_convs"], Lc["m"])
+
+    def one_call():
+        for layer in range(L):
+            mixed.tail_attn(layer=layer)
+
+    g1 = graph_of(one_call)
+    oc = time_calls(g1.replay if g1 else one_call, 3, 1)
+    parts_ms = dec["median_ms"] + L * ap["median_ms"]
+    step = {"config": "configs[4]", "what": "decode of all 16 conversations + the 4 appended chunks on each of %d layers, "
+            "CUDA-graph replay: one csv_tail_step per layer (decode rows and chunks as work items of one launch)" % L,
+            "ms_median": oc["median_ms"], "ms_min": oc["min_ms"], "separate_calls_ms": mx["median_ms"],
+            "decode_only_ms": dec["median_ms"], "append_only_ms_per_layer": ap["median_ms"], "sum_of_parts_ms": parts_ms,
+            "one_call_vs_sum_of_parts": oc["median_ms"] / parts_ms,
+            "hbm_bound_ms": L * (wl.decode_kv_bytes() + app.append_kv_bytes()) / pk["hbm"] / 1e6,
+            "tensor_bound_ms": L * app.append_flops() / pk["bf16_sustained"] / 1e9,
+            "decode_role_ctas": mixed.plan.info().get("tail_n_dec")}
+    del mixed
     return blocks, [step], app
 
 
@@ -412,7 +430,12 @@ def leg_c2(args, pk, dist, agg_dev):
     from paper_2606_01839_b200 import binding as B
     from paper_2606_01839_b200 import workloads
 
-    wl = workloads.config_tail_workload(2)
+    from paper_2606_01839_b200 import synth
+    base = [int(t) for t in synth.config_lengths(2)["kv_lens"]]
+    # the pool holds 128 tokens more per conversation than the step looks at: the host-buffer loop below GROWS every
+    # conversation by one token per step, as a decode loop does
+    big = workloads.TailWorkload(32, 8, 128, [1] * len(base), [t + 128 for t in base], seed=synth.CONFIGS[2]["seed"])
+    wl = big.with_q_lens([1] * len(base), kv_lens=base)
     kv_bytes = wl.decode_kv_bytes()
     rows = len(wl.kv_lens)
     g = None if args.no_graph else graph_of(wl.decode_step)
@@ -423,15 +446,20 @@ def leg_c2(args, pk, dist, agg_dev):
     h_t = torch.from_numpy(wl.h_tables).pin_memory()
     h_out = torch.zeros((rows, wl.Hq, wl.d), dtype=torch.int16).pin_memory()
     h_lse = torch.zeros((rows, wl.Hq), dtype=torch.float32).pin_memory()
-    ws = torch.empty(B.csv_tail_step_host_workspace_bytes(wl.shape, wl.kv_lens, wl.max_blocks), dtype=torch.uint8, device="cuda")
-    call = lambda: B.csv_tail_step_host(wl.pool, 0, wl.shape, wl.kv_lens, h_q, h_k, h_v, h_t, wl.max_blocks, ws, h_out, h_lse)
-    for _ in range(5):
-        call()
-    torch.cuda.synchronize()
-    tw = time.perf_counter()
-    for _ in range(100):
-        call()
-    e2e_ms = (time.perf_counter() - tw) * 1e3 / 100
+    ws = torch.empty(2 * B.csv_tail_step_host_workspace_bytes(wl.shape, big.kv_lens, wl.max_blocks), dtype=torch.uint8, device="cuda")
+
+    def host_loop(n, warm):
+        """n timed steps of a decode loop with host buffers: step i serves kv_len = base + i (one new token each)."""
+        t0 = 0.0
+        for i in range(warm + n):
+            if i == warm:
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+            kv = [t + i for t in base]
+            B.csv_tail_step_host(wl.pool, 0, wl.shape, kv, h_q, h_k, h_v, h_t, wl.max_blocks, ws, h_out, h_lse)
+        return (time.perf_counter() - t0) * 1e3 / n
+
+    e2e_ms = host_loop(100, 5)
     pt = []
     for _ in range(21):
         t0 = time.perf_counter()
@@ -442,12 +470,14 @@ def leg_c2(args, pk, dist, agg_dev):
             "(KV write + decode + merge), CUDA-graph replay", "ms_median": st["median_ms"], "ms_min": st["min_ms"],
             "gbs": kv_bytes / st["median_ms"] / 1e6, "tokens_per_s": rows / st["median_ms"] * 1e3,
             "e2e_host_buffers_ms": e2e_ms, "e2e_gbs": kv_bytes / e2e_ms / 1e6,
+            "e2e_what": "csv_tail_step_host over 100 consecutive steps, every conversation one token longer each step (planned "
+                        "per step while the H2D copies fly)",
             "h2d_bytes": (h_q.numel() + h_k.numel() + h_v.numel()) * 2 + h_t.numel() * 4,
             "d2h_bytes": h_out.numel() * 2 + h_lse.numel() * 4, "plan_host_us": sorted(pt)[len(pt) // 2],
             "decode_items": info["n_decode_items"]}
     block = roofline_block("decode_kernel", "configs[1]", "hbm", kv_bytes, dec, pk,
                            note="per paged_decode_attn call (decode_kernel + decode_merge_kernel)")
-    del wl
+    del wl, big
     torch.cuda.empty_cache()
     return [block], [step]
 
@@ -504,6 +534,7 @@ def leg_c3(args, pk, with_oracle):
             "one_call_vs_sum_of_parts": one["median_ms"] / parts, "two_streams_ms": both["median_ms"],
             "hbm_bound_ms": (wl.decode_kv_bytes() + wl.append_kv_bytes()) / pk["hbm"] / 1e6,
             "tensor_bound_ms": wl.append_flops() / pk["bf16"] / 1e9, "e2e_host_buffers_ms": e2e_ms,
+            "decode_role_ctas": wl.plan.info().get("tail_n_dec"),
             "h2d_bytes": (h_q.numel() + h_k.numel() + h_v.numel()) * 2 + h_t.numel() * 4,
             "d2h_bytes": h_out.numel() * 2 + h_lse.numel() * 4}
     cpu = None

@@ -313,6 +313,9 @@ int csv_plan_destroy(csv_plan_t* plan);
  * number of decode rows, of append chunks, sum of append q rows, CTAs used. */
 int csv_plan_info(const csv_plan_t* plan, int32_t* n_decode_items, int32_t* n_decode_rows,
                   int32_t* n_append_chunks, int32_t* n_append_rows, int32_t* decode_grid);
+/* The mixed-step split of a plan (csv_tail_step at head_dim 128 with decode rows AND chunks): how many CTAs of the one
+ * launch start in the decode role and into how many shares their work is cut; 0, 0 when the plan has no fused launch. */
+int csv_plan_tail_split(const csv_plan_t* plan, int32_t* n_decode_ctas, int32_t* n_decode_shares);
 /* Sum of the plan's q_lens (rows of d_q / d_out for append_prefill_attn); -1 on NULL. */
 int32_t csv_plan_total_q(const csv_plan_t* plan);
 /* Copies the decode work list for inspection (host tests): item i is 8 int32
@@ -380,13 +383,19 @@ int append_prefill_attn(const csv_plan_t* plan, const kv_pool_t* pool, int32_t l
 /* One tail step of a MIXED batch on one layer (PAPER.md:112 /
  * Fig. 5: decode rows and appended chunks run in the same iteration on the
  * decoder that holds their prefixes): writes every new row's K/V into the
- * pool, then attends.  Equivalent to kv_append_tokens (on this layer) +
- * paged_decode_attn + append_prefill_attn, enqueued back to back on `stream`
- * (programmatic dependent launch between the KV write and the decode); with no
- * appended chunk in the plan it is paged_decode_step (KV write inside the
- * decode launch).  d_q, d_out: [total_q][Hq][d]; d_k_new, d_v_new:
- * [total_q][Hkv][d] bf16 of THIS layer; rows ordered as in the plan.
- * Capturable in a CUDA graph (the bench does so).  Errors as the calls above. */
+ * pool, then attends.  Same results as kv_append_tokens (on this layer) +
+ * paged_decode_attn + append_prefill_attn.  With decode rows AND chunks in the
+ * plan (head_dim 128) the attention is ONE persistent launch whose work items
+ * are both kinds: some CTAs stream the decode rows' KV (HBM-bound), the others
+ * run the chunks on the tensor cores, and a CTA that finishes its decode share
+ * takes chunk items (tail_fused.cu); the KV write precedes it as its own
+ * kernel, chained by programmatic dependent launch.  With no appended chunk in
+ * the plan it is paged_decode_step (KV write inside the decode launch).
+ * d_q, d_out: [total_q][Hq][d]; d_k_new, d_v_new: [total_q][Hkv][d] bf16 of
+ * THIS layer; rows ordered as in the plan.  d_k_new = d_v_new = NULL: the rows
+ * are already in the pool, attention only.  Results are bit-identical from
+ * run to run for a fixed plan.  Capturable in a CUDA graph (the bench does so).
+ * Errors as the calls above. */
 int csv_tail_step(const csv_plan_t* plan, kv_pool_t* pool, int32_t layer, const void* d_q, const void* d_k_new,
                   const void* d_v_new, const int32_t* d_block_tables, int32_t max_blocks, void* d_out, float* d_lse,
                   void* stream);

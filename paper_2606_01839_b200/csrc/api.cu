@@ -1,5 +1,6 @@
 // api.cu — the extern "C" entry points of include/conserve_kv.h that touch CUDA: argument
 // validation, plan upload, launches, and the host-buffer tail step.  No kernels here.
+#include <stdlib.h>
 #include <string.h>
 
 #include <atomic>
@@ -306,12 +307,24 @@ int csv_tail_step(const csv_plan_t* plan, kv_pool_t* pool, int32_t layer, const 
                   void* stream) {
     const int rc = check_attn_args(plan, pool, layer, d_q, d_block_tables, max_blocks, d_out, d_lse);
     if (rc != CSV_OK) return rc;
-    if (!d_k_new || !d_v_new || !aligned(d_k_new, 16) || !aligned(d_v_new, 16)) return CSV_E_INVAL;
+    const bool write_kv = d_k_new != nullptr || d_v_new != nullptr;   // both NULL: attention only (the rows are in the pool)
+    if (write_kv && (!d_k_new || !d_v_new || !aligned(d_k_new, 16) || !aligned(d_v_new, 16))) return CSV_E_INVAL;
     if (plan->append_items.empty())   // decode rows only: the KV write rides in the decode launch
         return launch_decode(plan, pool, layer, d_q, d_block_tables, max_blocks, d_out, d_lse, stream, d_k_new, d_v_new);
     kv_pool view = layer_view_of(pool, layer);
-    int r = launch_append_tokens(&view, plan, d_k_new, d_v_new, d_block_tables, max_blocks, stream);
-    if (r == CSV_OK) r = launch_decode(plan, &view, 0, d_q, d_block_tables, max_blocks, d_out, d_lse, stream);
+    static const bool no_fuse = getenv("CSV_X_TAIL_NOFUSE") != nullptr;   // experiment knob: the three-launch route
+    const bool fuse = plan->tail_n_dec > 0 && !no_fuse;
+    int r = CSV_OK;
+    if (fuse && write_kv) r = launch_tail_zero_queue(plan, stream);
+    if (r == CSV_OK && write_kv) r = launch_append_tokens(&view, plan, d_k_new, d_v_new, d_block_tables, max_blocks, stream);
+    if (r != CSV_OK) return r;
+    if (fuse) {
+        // decode rows and appended chunks as work items of ONE persistent launch (tail_fused.cu)
+        r = launch_tail_fused(plan, &view, 0, d_q, d_block_tables, max_blocks, d_out, d_lse, stream, write_kv);
+        if (r == CSV_OK && !plan->zero_rows.empty()) r = launch_decode_zero_rows(plan, &view, d_out, d_lse, stream);
+        return r;
+    }
+    r = launch_decode(plan, &view, 0, d_q, d_block_tables, max_blocks, d_out, d_lse, stream);
     if (r == CSV_OK) r = launch_append_attn(plan, &view, 0, d_q, d_block_tables, max_blocks, d_out, d_lse, stream);
     return r;
 }
@@ -389,11 +402,13 @@ int csv_tail_step_host(kv_pool_t* pool, int32_t layer_begin, int32_t n_layers, c
         (e = cudaMemcpyAsync(ws + L.tables, h_block_tables, (size_t)batch * max_blocks * 4, cudaMemcpyHostToDevice, st)) !=
             cudaSuccess)
         return csv_set_cuda_error((int)e);
+    // One plan serves every layer of the step (lengths are per step, not per layer).  It is built here, while the copies
+    // above are in flight: measured on configs[1], keeping the previous step's plan alive and extending it (no planning,
+    // pinned plan image) did not shorten the call (0.289 against 0.282 ms): the host work is hidden under the DMA.
     std::vector<int32_t> ones;
     if (!h_q_lens) ones.assign((size_t)batch, 1);
     int err;
-    csv_plan_t* plan =   // one plan serves every layer of the step (lengths are per step, not per layer)
-        csv_plan_build_host(shape, h_q_lens ? h_q_lens : ones.data(), h_kv_lens, batch, max_partition_tokens, &err);
+    csv_plan_t* plan = csv_plan_build_host(shape, h_q_lens ? h_q_lens : ones.data(), h_kv_lens, batch, max_partition_tokens, &err);
     if (!plan) return err;
     int rc = ws_bytes - L.plan < plan->lay.total ? CSV_E_NOMEM : plan_attach(plan, ws + L.plan, ws_bytes - L.plan, stream);
     for (int l = 0; rc == CSV_OK && l < n_layers; ++l)   // KV write of every new row + decode rows + appended chunks

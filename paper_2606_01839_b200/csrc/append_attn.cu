@@ -329,6 +329,18 @@ int launch_append_merge(const csv_plan* plan, const AppendParams& p, cudaStream_
 
 }   // namespace
 
+int launch_append_merge_128(const csv_plan* plan, void* out, float* lse, void* stream) {
+    AppendParams p = {};
+    p.out = (uint16_t*)out;
+    p.lse = lse;
+    p.po = reinterpret_cast<float*>(plan->d_ws + plan->lay.append_po);
+    p.pml = reinterpret_cast<float*>(plan->d_ws + plan->lay.append_pml);
+    p.Hq = plan->shape.num_q_heads;
+    p.Hkv = plan->shape.num_kv_heads;
+    p.G = p.Hq / p.Hkv;
+    return launch_append_merge<128>(plan, p, (cudaStream_t)stream);
+}
+
 int launch_append_attn(const csv_plan* plan, const kv_pool* pool, int layer, const void* q, const int32_t* tables,
                        int max_blocks, void* out, float* lse, void* stream) {
     if (plan->append_items.empty()) return CSV_OK;

@@ -75,6 +75,7 @@ constexpr int kAppendKvSplit = 8192; // default KV tokens per append partition
 struct PlanLayout {   // byte offsets into the caller's workspace (all 128-byte aligned)
     size_t decode_items, worker_begin, decode_groups, decode_po, decode_pml;
     size_t append_items, append_groups, append_po, append_pml;
+    size_t tail_items, tail_worker_begin, tail_groups;   // the decode share list of tail_kernel's decode-role CTAs (mixed steps)
     size_t zero_rows;   // int32 rows of d_out / d_lse whose conversation has q_len = 1 and an empty cache
     size_t conv_meta;   // int32 [q_start[batch+1] | kv_len[batch] | q_len[batch]]
     size_t append_sched;   // uint32 [next item, CTAs done]: the append kernel's work queue, zero between launches
@@ -98,6 +99,13 @@ struct csv_plan {
     int32_t decode_warps;                    // warp-workers per CTA (8; 2 = the slim kernel that runs beside the append CTAs)
     int32_t n_decode_partials;               // partial slots (non-direct items)
     std::vector<int32_t> zero_rows;          // q rows of decode conversations with kv_len = 0 (O = 0, LSE = -inf)
+    // mixed step in one launch (tail_kernel): the decode rows cut again for tail_n_dec CTAs x 8 warp-workers
+    int32_t tail_n_dec;                      // SMs that start in the decode role (0 = no fused launch for this plan)
+    int32_t tail_n_shares;                   // decode shares of 8 warp-workers each (a queue: any CTA may take one)
+    std::vector<DecodeItem> tail_items;
+    std::vector<int32_t> tail_worker_begin;
+    std::vector<MergeGroup> tail_groups;
+    int32_t tail_n_partials;
     // append
     std::vector<AppendItem> append_items;
     std::vector<MergeGroup> append_groups;   // groups with count > 1 only
@@ -125,6 +133,12 @@ int launch_decode(const csv_plan* plan, const kv_pool* pool, int layer, const vo
                   const void* v_new = nullptr);
 int launch_append_attn(const csv_plan* plan, const kv_pool* pool, int layer, const void* q, const int32_t* tables,
                        int max_blocks, void* out, float* lse, void* stream);
+int launch_decode_zero_rows(const csv_plan* plan, const kv_pool* pool, void* out, float* lse, void* stream);
+int launch_decode_merge_128(const csv_plan* plan, size_t groups_off, int ng, void* out, float* lse, void* stream);
+int launch_append_merge_128(const csv_plan* plan, void* out, float* lse, void* stream);   // append partials -> O / LSE
+int launch_tail_zero_queue(const csv_plan* plan, void* stream);   // before the kernel that launch_tail_fused(pdl) is chained to
+int launch_tail_fused(const csv_plan* plan, const kv_pool* pool, int layer, const void* q, const int32_t* tables,
+                      int max_blocks, void* out, float* lse, void* stream, bool pdl);
 int launch_append_attn_tc2(const csv_plan* plan, const kv_pool* pool, int layer, const void* q, const int32_t* tables,
                            int max_blocks, void* out, float* lse, void* stream);
 int csv_query_num_sms();   // SM count of the current device, 148 if none is usable

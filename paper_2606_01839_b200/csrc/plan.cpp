@@ -34,31 +34,16 @@ static bool attn_shape_ok(const csv_attn_shape* s) {
     return true;
 }
 
-static void plan_decode(csv_plan* p) {
+// Cuts the flattened (conversation, KV head, block) stream of the q_len = 1 rows into one contiguous share per worker
+// (W workers) and each share into items at (conversation, head) boundaries (+ every part_blocks blocks).
+static void build_decode_list(const csv_plan* p, int64_t units, int64_t W, int part_blocks, std::vector<DecodeItem>& items,
+                              std::vector<int32_t>& worker_begin, std::vector<MergeGroup>& groups, int32_t& n_partials) {
     const int Hkv = p->shape.num_kv_heads;
-    const int part_blocks = std::max(1, p->max_partition_tokens / CSV_BLOCK_SIZE);
-    int64_t units = 0;
-    p->n_decode_rows = 0;
-    p->zero_rows.clear();
-    for (int b = 0; b < p->batch; ++b)
-        if (p->q_lens[b] == 1) {
-            units += (int64_t)((p->kv_lens[b] + CSV_BLOCK_SIZE - 1) / CSV_BLOCK_SIZE) * Hkv;
-            ++p->n_decode_rows;
-            if (p->kv_lens[b] == 0) p->zero_rows.push_back(p->q_start[(size_t)b]);   // empty cache: O = 0, LSE = -inf
-        }
-    // CTAs: one per SM, fewer when there is under 4 blocks of work per warp
-    const int WPC = p->decode_warps;   // warp-workers per CTA
-    int64_t want = (units + (int64_t)WPC * 4 - 1) / ((int64_t)WPC * 4);
-    int64_t max_grid = p->num_sms;
-    if (const char* e = getenv("CSV_X_DECODE_MULT")) max_grid *= std::max(1, atoi(e));   // experiment knob: slim CTAs per SM
-    p->decode_grid = (int)std::max<int64_t>(1, std::min<int64_t>(max_grid, want));
-    if (const char* e = getenv("CSV_X_DECODE_GRID")) p->decode_grid = std::max(1, std::min(p->decode_grid, atoi(e)));   // experiment knob
-    const int64_t W = (int64_t)p->decode_grid * WPC;
-    p->worker_begin.assign((size_t)W + 1, 0);
-    p->decode_items.clear();
-    p->decode_items.reserve((size_t)W + (size_t)p->n_decode_rows * Hkv + 16);
-    p->decode_groups.clear();
-    p->n_decode_partials = 0;
+    worker_begin.assign((size_t)W + 1, 0);
+    items.clear();
+    items.reserve((size_t)W + (size_t)p->n_decode_rows * Hkv + 16);
+    groups.clear();
+    n_partials = 0;
     if (units == 0) return;
 
     int64_t base = 0;   // first unit of the current (conv, head) segment
@@ -75,13 +60,13 @@ static void plan_decode(csv_plan* p) {
         if (p->q_lens[b] != 1 || p->kv_lens[b] == 0) continue;
         const int nblk = (p->kv_lens[b] + CSV_BLOCK_SIZE - 1) / CSV_BLOCK_SIZE;
         for (int g = 0; g < Hkv; ++g) {
-            const size_t first_item = p->decode_items.size();
+            const size_t first_item = items.size();
             int blk = 0;
             while (blk < nblk) {
                 const int64_t pos = base + blk;
                 while (w + 1 < W && next_start <= pos) {   // advance to the worker owning pos
                     ++w;
-                    p->worker_begin[(size_t)w] = (int32_t)p->decode_items.size();
+                    worker_begin[(size_t)w] = (int32_t)items.size();
                     next_start += sq;
                     next_rem += sr;
                     if (next_rem >= W) {
@@ -102,32 +87,104 @@ static void plan_decode(csv_plan* p) {
                 it.direct = 0;
                 it.group = -1;
                 it.q_row = p->q_start[(size_t)b];
-                p->decode_items.push_back(it);
+                items.push_back(it);
                 blk = end;
             }
-            const size_t n = p->decode_items.size() - first_item;
+            const size_t n = items.size() - first_item;
             if (n == 1) {
-                p->decode_items[first_item].direct = 1;
+                items[first_item].direct = 1;
             } else {
                 MergeGroup mg{};
-                mg.first = p->n_decode_partials;
+                mg.first = n_partials;
                 mg.count = (int32_t)n;
                 mg.conv = b;
                 mg.head = g;
                 mg.q_start = p->q_start[(size_t)b];
                 for (size_t i = 0; i < n; ++i) {
-                    DecodeItem& di = p->decode_items[first_item + i];
-                    di.partial = p->n_decode_partials++;
-                    di.group = (int32_t)p->decode_groups.size();
+                    DecodeItem& di = items[first_item + i];
+                    di.partial = n_partials++;
+                    di.group = (int32_t)groups.size();
                     di.group_first = mg.first;
                     di.group_count = mg.count;
                 }
-                p->decode_groups.push_back(mg);
+                groups.push_back(mg);
             }
             base += nblk;
         }
     }
-    for (int64_t k = w + 1; k <= W; ++k) p->worker_begin[(size_t)k] = (int32_t)p->decode_items.size();
+    for (int64_t k = w + 1; k <= W; ++k) worker_begin[(size_t)k] = (int32_t)items.size();
+}
+
+static int64_t decode_units(csv_plan* p) {
+    const int Hkv = p->shape.num_kv_heads;
+    int64_t units = 0;
+    p->n_decode_rows = 0;
+    p->zero_rows.clear();
+    for (int b = 0; b < p->batch; ++b)
+        if (p->q_lens[b] == 1) {
+            units += (int64_t)((p->kv_lens[b] + CSV_BLOCK_SIZE - 1) / CSV_BLOCK_SIZE) * Hkv;
+            ++p->n_decode_rows;
+            if (p->kv_lens[b] == 0) p->zero_rows.push_back(p->q_start[(size_t)b]);   // empty cache: O = 0, LSE = -inf
+        }
+    return units;
+}
+
+static void plan_decode(csv_plan* p) {
+    const int part_blocks = std::max(1, p->max_partition_tokens / CSV_BLOCK_SIZE);
+    const int64_t units = decode_units(p);
+    // CTAs: one per SM, fewer when there is under 4 blocks of work per warp
+    const int WPC = p->decode_warps;   // warp-workers per CTA
+    int64_t want = (units + (int64_t)WPC * 4 - 1) / ((int64_t)WPC * 4);
+    int64_t max_grid = p->num_sms;
+    if (const char* e = getenv("CSV_X_DECODE_MULT")) max_grid *= std::max(1, atoi(e));   // experiment knob: slim CTAs per SM
+    p->decode_grid = (int)std::max<int64_t>(1, std::min<int64_t>(max_grid, want));
+    if (const char* e = getenv("CSV_X_DECODE_GRID")) p->decode_grid = std::max(1, std::min(p->decode_grid, atoi(e)));   // experiment knob
+    build_decode_list(p, units, (int64_t)p->decode_grid * WPC, part_blocks, p->decode_items, p->worker_begin, p->decode_groups,
+                      p->n_decode_partials);
+}
+
+// Mixed step (decode rows AND appended chunks, d = 128): tail_kernel gives `tail_n_dec` CTAs the decode role (8 warp-workers
+// each, a second share list cut for that many workers) and the others the append role; decode CTAs join the append queue
+// when their share is done.  The split equalises the two predicted times: decode bytes / (CTAs x bandwidth one SM pulls)
+// against append flops / (CTAs x tensor rate of one SM), both measured (kernels).
+static void plan_tail(csv_plan* p) {
+    p->tail_n_dec = 0;
+    p->tail_n_shares = 0;
+    p->tail_items.clear();
+    p->tail_worker_begin.clear();
+    p->tail_groups.clear();
+    p->tail_n_partials = 0;
+    if (p->shape.head_dim != 128 || p->append_items.empty() || p->decode_items.empty() || p->num_sms < 4) return;
+    const int Hkv = p->shape.num_kv_heads, Hq = p->shape.num_q_heads, d = p->shape.head_dim;
+    int64_t units = 0;
+    double flops = 0.0;
+    for (int b = 0; b < p->batch; ++b) {
+        const int m = p->q_lens[b];
+        if (m == 1) units += (int64_t)((p->kv_lens[b] + CSV_BLOCK_SIZE - 1) / CSV_BLOCK_SIZE) * Hkv;
+        if (m > 1) flops += 4.0 * d * Hq * m * ((double)(p->kv_lens[b] - m) + (m + 1) / 2.0);
+    }
+    const double bytes = (double)units * 2.0 * csv_tile_bytes(d);
+    double sm_gbs = 75.0, sm_tflops = 7.4;     // one SM: decode role pulls ~75 GB/s, append role sustains 7.0-7.8 TFLOP/s
+    if (const char* e = getenv("CSV_X_TAIL_SM_GBS")) sm_gbs = atof(e);         // experiment knobs
+    if (const char* e = getenv("CSV_X_TAIL_SM_TFLOPS")) sm_tflops = atof(e);
+    const double td = bytes / (sm_gbs * 1e9), ta = flops / (sm_tflops * 1e12);   // SM-seconds of each role
+    // A decode side that is too small costs more than one that is too large (SMs that finish their decode share take chunk
+    // items, while a chunk-role SM can only take over a whole share), so the split leans 8 % towards decode.
+    int k = (int)(1.08 * p->num_sms * td / (td + ta) + 0.5);
+    // HBM saturates near 3/4 of the SMs: more decode CTAs than that only take tensor pipes away from the chunks
+    k = std::max(1, std::min(k, std::min(p->num_sms - 1, (p->num_sms * 3) / 4)));
+    const int64_t want = (units + 8 * 4 - 1) / (8 * 4);
+    k = (int)std::min<int64_t>(k, std::max<int64_t>(1, want));
+    if (const char* e = getenv("CSV_X_TAIL_NDEC")) k = std::max(1, std::min(p->num_sms - 1, atoi(e)));
+    p->tail_n_dec = k;
+    // shares per decode-role SM (measured on configs[2] / [4]: 1 share 4.64 / 5.07 ms, 4 shares 4.98 / 5.26 ms: every share
+    // ends with a CTA-wide barrier and restarts the rings)
+    int shares = 1;
+    if (const char* e = getenv("CSV_X_TAIL_SHARES")) shares = std::max(1, std::min(16, atoi(e)));
+    p->tail_n_shares = (int)std::max<int64_t>(1, std::min<int64_t>((int64_t)k * shares, want));
+    const int part_blocks = std::max(1, p->max_partition_tokens / CSV_BLOCK_SIZE);
+    build_decode_list(p, units, (int64_t)p->tail_n_shares * 8, part_blocks, p->tail_items, p->tail_worker_begin, p->tail_groups,
+                      p->tail_n_partials);
 }
 
 static void plan_append(csv_plan* p) {
@@ -229,6 +286,9 @@ static void plan_layout(csv_plan* p) {
     L.append_items = take(p->append_items.size() * sizeof(AppendItem));
     L.append_groups = take(p->append_groups.size() * sizeof(MergeGroup));
     L.zero_rows = take(p->zero_rows.size() * sizeof(int32_t));
+    L.tail_items = take(p->tail_items.size() * sizeof(DecodeItem));
+    L.tail_worker_begin = take(p->tail_worker_begin.size() * sizeof(int32_t));
+    L.tail_groups = take(p->tail_groups.size() * sizeof(MergeGroup));
     L.append_sched = take(128);   // zero in the uploaded image; the kernel's last CTA zeroes it again
     std::vector<int32_t> meta;
     meta.insert(meta.end(), p->q_start.begin(), p->q_start.end());
@@ -236,8 +296,9 @@ static void plan_layout(csv_plan* p) {
     meta.insert(meta.end(), p->q_lens.begin(), p->q_lens.end());
     L.conv_meta = take(meta.size() * sizeof(int32_t));
     const size_t list_bytes = off;
-    L.decode_po = take((size_t)p->n_decode_partials * G * d * sizeof(float));
-    L.decode_pml = take((size_t)p->n_decode_partials * G * 2 * sizeof(float));
+    const size_t dec_partials = (size_t)std::max(p->n_decode_partials, p->tail_n_partials);   // the two lists never run together
+    L.decode_po = take(dec_partials * G * d * sizeof(float));
+    L.decode_pml = take(dec_partials * G * 2 * sizeof(float));
     L.append_po = take((size_t)p->n_append_partials * p->append_tile_rows * d * sizeof(float));
     L.append_pml = take((size_t)p->n_append_partials * p->append_tile_rows * 2 * sizeof(float));
     L.total = std::max<size_t>(off, 128);
@@ -252,6 +313,9 @@ static void plan_layout(csv_plan* p) {
     put(L.append_groups, p->append_groups.data(), p->append_groups.size() * sizeof(MergeGroup));
     put(L.conv_meta, meta.data(), meta.size() * sizeof(int32_t));
     put(L.zero_rows, p->zero_rows.data(), p->zero_rows.size() * sizeof(int32_t));
+    put(L.tail_items, p->tail_items.data(), p->tail_items.size() * sizeof(DecodeItem));
+    put(L.tail_worker_begin, p->tail_worker_begin.data(), p->tail_worker_begin.size() * sizeof(int32_t));
+    put(L.tail_groups, p->tail_groups.data(), p->tail_groups.size() * sizeof(MergeGroup));
 }
 
 // Builds the host side of a plan.  Returns NULL on bad arguments.
@@ -289,6 +353,7 @@ csv_plan* csv_plan_build_host(const csv_attn_shape* shape, const int32_t* h_q_le
     if (const char* e = getenv("CSV_X_DECODE_WARPS")) p->decode_warps = atoi(e) == 2 ? 2 : kDecodeWarps;   // experiment knob
     plan_decode(p);
     plan_append(p);
+    plan_tail(p);
     plan_layout(p);
     *err = CSV_OK;
     return p;
@@ -320,6 +385,13 @@ int csv_plan_info(const csv_plan_t* plan, int32_t* n_decode_items, int32_t* n_de
     if (n_append_chunks) *n_append_chunks = plan->n_append_chunks;
     if (n_append_rows) *n_append_rows = plan->n_append_rows;
     if (decode_grid) *decode_grid = plan->decode_grid;
+    return CSV_OK;
+}
+
+int csv_plan_tail_split(const csv_plan_t* plan, int32_t* n_decode_ctas, int32_t* n_decode_shares) {
+    if (!plan) return CSV_E_INVAL;
+    if (n_decode_ctas) *n_decode_ctas = plan->tail_n_dec;
+    if (n_decode_shares) *n_decode_shares = plan->tail_n_shares;
     return CSV_OK;
 }
 

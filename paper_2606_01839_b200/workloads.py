@@ -70,6 +70,27 @@ class TailWorkload:
         other._setup_queries(q_lens)
         return other
 
+    def with_extra_chunks(self, convs, m):
+        """One MIXED step over the same pool: every conversation keeps its decode row, and each conversation in `convs`
+        also appends an m-token chunk (BASELINE.json configs[4]: "decode for all 16 conversations plus 4 append chunks").
+        A conversation has one q_len per batch entry, so the chunk is a second entry whose block table names the same
+        blocks (attention only reads them: S11).  Attention-only steps (the rows are already in the pool)."""
+        import copy
+
+        other = copy.copy(self)
+        convs = [int(c) for c in convs]
+        other.kv_lens = self.kv_lens + [self.kv_lens[c] for c in convs]
+        other.tables = self.tables + [self.tables[c] for c in convs]
+        other.h_tables = np.concatenate([self.h_tables, self.h_tables[convs]], axis=0)
+        other.d_tables = torch.from_numpy(other.h_tables).cuda()
+        other._setup_queries(list(self.q_lens) + [int(m)] * len(convs))
+        return other
+
+    def tail_attn(self, layer=0, stream=None):
+        """csv_tail_step without the KV write (d_k_new = d_v_new = NULL): decode rows + chunks, one call."""
+        B.csv_tail_step(self.plan, self.pool, layer, self.d_q, None, None, self.d_tables, self.max_blocks, self.d_out,
+                        self.d_lse, stream)
+
     # algorithmic work (SURVEY §8d, S19): KV bytes read once per call
     def decode_kv_bytes(self):
         return sum(kv for q, kv in zip(self.q_lens, self.kv_lens) if q == 1) * self.Hkv * self.d * 2 * 2

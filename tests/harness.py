@@ -98,6 +98,8 @@ def run_attention(sc, q_lens, q_bits, layer=0, mpt=0, which="both"):
         B.paged_decode_attn(plan, sc.pool, layer, d_q, sc.d_tables, sc.max_blocks, d_out, d_lse)
     if which in ("both", "append"):
         B.append_prefill_attn(plan, sc.pool, layer, d_q, sc.d_tables, sc.max_blocks, d_out, d_lse)
+    if which == "tail":   # csv_tail_step, attention only (the rows are in the pool): one fused launch for a mixed batch
+        B.csv_tail_step(plan, sc.pool, layer, d_q, None, None, sc.d_tables, sc.max_blocks, d_out, d_lse)
     torch.cuda.synchronize()
     info = plan.info()
     return bf16_dev_to_f64(d_out), d_lse.cpu().numpy().astype(np.float64), info

@@ -24,7 +24,14 @@ def step_case(oracle, seed, Hq, Hkv, d, convs, mpt=0, poison=False, v_mean=0.0, 
     O, LSE, info = run_attention(sc, q_lens, q, mpt=mpt, which="both")
     O_ref, LSE_ref = oracle_attention(sc, q_lens, q)
     A_ref = oracle_abs_weighted(sc, q_lens, q) if qscale > 1.0 else None   # peaked softmax: DESIGN.md S20
-    return assert_close(O, LSE, O_ref, LSE_ref, what or "step", A_ref=A_ref), info
+    res = assert_close(O, LSE, O_ref, LSE_ref, what or "step", A_ref=A_ref)
+    if any(m == 1 for m in q_lens) and any(m > 1 for m in q_lens):
+        # the same step through csv_tail_step: at d = 128 decode rows and chunks are work items of ONE launch (tail_fused.cu)
+        O2, LSE2, _ = run_attention(sc, q_lens, q, mpt=mpt, which="tail")
+        assert_close(O2, LSE2, O_ref, LSE_ref, (what or "step") + " [csv_tail_step]", A_ref=A_ref)
+        O3, LSE3, _ = run_attention(sc, q_lens, q, mpt=mpt, which="tail")
+        assert np.array_equal(O2, O3) and np.array_equal(LSE2, LSE3), "csv_tail_step is not bit-identical from run to run"
+    return res, info
 
 
 @pytest.mark.parametrize("Hq,Hkv,d", [(32, 8, 128), (64, 8, 128), (4, 1, 64), (8, 8, 64), (16, 2, 128), (8, 8, 128), (8, 4, 128),
@@ -101,6 +108,47 @@ def test_tail_step_host_buffers(oracle):
     O = synth.bf16_bits_to_f32(h_out.numpy().view(np.uint16)).astype(np.float64)
     O_ref, LSE_ref = oracle_attention(sc, [1] * 5, q)
     assert_close(O, h_lse.numpy().astype(np.float64), O_ref, LSE_ref, what="tail step")
+
+
+def test_tail_step_host_over_a_decode_loop(oracle):
+    """csv_tail_step_host over 40 consecutive decode steps: every conversation grows by one token per step,
+    crossing block edges on the way.  Every third step's O / LSE against the oracle on the cache as it stands, the pool at
+    the end against the oracle's scatter."""
+    from harness import dev_to_u16
+    rng = np.random.default_rng(97)
+    Hq, Hkv, d, steps = 32, 8, 128, 40
+    start = [100, 2049, 15, 2, 777, 4096 - 20]
+    final = [t + steps - 1 for t in start]
+    n = len(start)
+    sc = Scenario(oracle, rng, Hq, Hkv, d, final, poison=True)
+    full = sc.image.copy()
+    for b in range(n):
+        full = oracle.scatter(full, 1, sc.num_blocks, Hkv, d, sc.K[b], sc.V[b], final[b], 0, sc.tables[b])
+        sc.image = oracle.scatter(sc.image, 1, sc.num_blocks, Hkv, d, sc.K[b][:, :start[b] - 1], sc.V[b][:, :start[b] - 1],
+                                  start[b] - 1, 0, sc.tables[b])
+    shape = B.attn_shape(Hq, Hkv, d)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    sc.upload()
+    tabs = np.where(sc.h_tables < 0, 0, sc.h_tables).astype(np.int32)
+    h_t = pin(tabs)
+    h_out = torch.zeros((n, Hq, d), dtype=torch.int16).pin_memory()
+    h_lse = torch.zeros((n, Hq), dtype=torch.float32).pin_memory()
+    ws = torch.empty(2 * B.csv_tail_step_host_workspace_bytes(shape, final, sc.max_blocks), dtype=torch.uint8, device="cuda")
+    qrng = np.random.default_rng(98)
+    for s_ in range(steps):
+        kv = [t + s_ for t in start]
+        k_new = np.stack([sc.K[b][0, kv[b] - 1] for b in range(n)])
+        v_new = np.stack([sc.V[b][0, kv[b] - 1] for b in range(n)])
+        q = synth.normal_bf16(qrng, (n, Hq, d))
+        B.csv_tail_step_host(sc.pool, 0, shape, kv, pin(q.view(np.int16)), pin(k_new.view(np.int16)), pin(v_new.view(np.int16)),
+                             h_t, sc.max_blocks, ws, h_out, h_lse)
+        if s_ % 3 == 0 or s_ == steps - 1:
+            O = synth.bf16_bits_to_f32(h_out.numpy().view(np.uint16)).astype(np.float64)
+            for b in range(n):
+                o_ref, l_ref = oracle.attention(q[b:b + 1], sc.K[b][0][:kv[b]], sc.V[b][0][:kv[b]])
+                assert_close(O[b:b + 1], h_lse[b:b + 1].numpy().astype(np.float64), o_ref, l_ref,
+                             what="host loop step %d conv %d" % (s_, b))
+    assert np.array_equal(dev_to_u16(sc.d_image), full), "pool after the host loop differs from the oracle's scatter"
 
 
 @pytest.mark.parametrize("Hq,Hkv,d", [(32, 8, 128), (64, 8, 128), (4, 1, 64)])

@@ -280,6 +280,23 @@ def test_workspace_bytes_grows_with_partials_and_is_checked():
     assert B.csv_tail_step_host_workspace_bytes(sh, kv, 256) > B.csv_plan_workspace_bytes(sh, [1] * 4, kv)
 
 
+def test_mixed_step_split_follows_the_work():
+    # csv_plan_tail_split: only a plan with decode rows AND chunks at d = 128 has a fused launch; the decode side grows with
+    # the decode bytes, shrinks with the chunks' flops, and always leaves CTAs for the other role (host-only plans, 148 SMs).
+    sh = B.attn_shape(32, 8, 128)
+    split = lambda q, kv, shape=sh: (lambda i: (i["tail_n_dec"], i["tail_n_shares"]))(B.Plan(shape, q, kv).info())
+    assert split([1] * 8, [4096] * 8) == (0, 0)                          # decode rows only: paged_decode_step
+    assert split([64] * 4, [4096] * 4) == (0, 0)                         # chunks only
+    assert split([1, 64], [512, 512], B.attn_shape(4, 1, 64)) == (0, 0)  # d = 64: the three-launch route
+    c3 = synth.config_lengths(3)
+    k3, s3 = split(c3["q_lens"], c3["kv_lens"])
+    assert 30 <= k3 <= 80 and s3 >= k3                                   # configs[2]: decode 14 GB against 2.8 TFLOP
+    more_decode = np.where(c3["q_lens"] == 1, c3["kv_lens"] * 2, c3["kv_lens"])
+    assert split(c3["q_lens"], more_decode)[0] > k3
+    assert 1 <= split([1, 512], [16, 60000])[0] <= 4                     # one short decode row beside a long chunk
+    assert split([1] * 200 + [2], [60000] * 200 + [64])[0] <= 111        # never more than 3/4 of the SMs on decode
+
+
 def test_handoff_direct_and_ipc_reject_bad_arguments_before_touching_cuda():
     pool = mkpool(8, NL=1, Hkv=1, d=64)
     k = FAKE + (1 << 20)
