@@ -313,6 +313,9 @@ int csv_plan_destroy(csv_plan_t* plan);
  * number of decode rows, of append chunks, sum of append q rows, CTAs used. */
 int csv_plan_info(const csv_plan_t* plan, int32_t* n_decode_items, int32_t* n_decode_rows,
                   int32_t* n_append_chunks, int32_t* n_append_rows, int32_t* decode_grid);
+/* Warp-workers of the decode launch = rows of h_worker_begin minus one (CTAs x workers per CTA: 7 at head_dim 128, 8 at 64). */
+int32_t csv_plan_decode_workers(const csv_plan_t* plan);
+
 /* The mixed-step split of a plan (csv_tail_step at head_dim 128 with decode rows AND chunks): how many CTAs of the one
  * launch start in the decode role and into how many shares their work is cut; 0, 0 when the plan has no fused launch. */
 int csv_plan_tail_split(const csv_plan_t* plan, int32_t* n_decode_ctas, int32_t* n_decode_shares);

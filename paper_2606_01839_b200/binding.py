@@ -21,7 +21,7 @@ SYMBOLS = [
     "kv_pool_set_free_order", "kv_alloc_blocks", "kv_free_blocks", "kv_pool_used_blocks", "kv_pool_num_blocks",
     "kv_pool_free_blocks", "kv_pool_get_desc", "csv_place", "csv_provision", "kv_staging_bytes", "kv_pack",
     "kv_unpack", "kv_pack_batch", "kv_unpack_batch", "kv_append_tokens", "csv_plan_workspace_bytes",
-    "csv_plan_create", "csv_plan_destroy", "csv_plan_info", "csv_plan_tail_split", "csv_plan_total_q", "csv_plan_decode_items",
+    "csv_plan_create", "csv_plan_destroy", "csv_plan_info", "csv_plan_tail_split", "csv_plan_decode_workers", "csv_plan_total_q", "csv_plan_decode_items",
     "csv_plan_append_items", "paged_decode_attn", "paged_decode_step", "append_prefill_attn", "csv_tail_step_host_workspace_bytes",
     "csv_tail_step_host", "kv_handoff_direct", "kv_handoff_direct_batch", "csv_ipc_export", "csv_ipc_open", "csv_ipc_close", "csv_ipc_copy", "csv_tail_step",
 ]
@@ -91,6 +91,7 @@ def lib():
             "csv_plan_destroy": (ctypes.c_int, [vp]),
             "csv_plan_info": (ctypes.c_int, [vp, pi32, pi32, pi32, pi32, pi32]),
             "csv_plan_tail_split": (ctypes.c_int, [vp, pi32, pi32]),
+            "csv_plan_decode_workers": (i32, [vp]),
             "csv_plan_total_q": (i32, [vp]),
             "csv_plan_decode_items": (i32, [vp, pi32, i32, pi32, i32]),
             "csv_plan_append_items": (i32, [vp, pi32, i32]),
@@ -348,7 +349,7 @@ class Plan:
         out = dict(zip(keys, [x.value for x in v]))
         a, b = ctypes.c_int32(), ctypes.c_int32()
         _check("csv_plan_tail_split", lib().csv_plan_tail_split(self.handle, ctypes.byref(a), ctypes.byref(b)))
-        out.update(tail_n_dec=a.value, tail_n_shares=b.value)
+        out.update(tail_n_dec=a.value, tail_n_shares=b.value, decode_workers=int(lib().csv_plan_decode_workers(self.handle)))
         return out
 
     @property
@@ -357,7 +358,7 @@ class Plan:
 
     def decode_items(self):
         inf = self.info()
-        n, W = inf["n_decode_items"], inf["decode_grid"] * 8
+        n, W = inf["n_decode_items"], inf["decode_workers"]
         items = np.zeros((max(n, 1), 8), dtype=np.int32)
         wb = np.zeros(W + 1, dtype=np.int32)
         lib().csv_plan_decode_items(self.handle, items.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)), n,

@@ -75,7 +75,7 @@ __global__ void decode_zero_rows_kernel(const int32_t* __restrict__ rows, int ro
 }
 
 template <int D, int STAGES, int WARPS>
-__global__ void __launch_bounds__(WARPS * 32, WARPS == 8 ? 1 : 512 / (WARPS * 32)) decode_kernel(const __grid_constant__ DecodeParams p) {
+__global__ void __launch_bounds__(WARPS * 32, WARPS >= 4 ? 1 : 512 / (WARPS * 32)) decode_kernel(const __grid_constant__ DecodeParams p) {
     constexpr int TB = 16 * D * 2;   // tile bytes
     extern __shared__ __align__(1024) uint8_t smem[];
     const int warp = threadIdx.x >> 5;
@@ -93,7 +93,7 @@ int launch_decode_t(const csv_plan* plan, const DecodeParams& p, cudaStream_t st
     CSV_CUDA_TRY(once_per_device(attr, [&] {
         cudaError_t e = cudaFuncSetAttribute(decode_kernel<D, STAGES, WARPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         // the slim variant runs BESIDE the append CTA: the SM must be carved for both kernels' shared memory at once
-        if (e == cudaSuccess && WARPS != 8)
+        if (e == cudaSuccess && WARPS < 4)
             e = cudaFuncSetAttribute(decode_kernel<D, STAGES, WARPS>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
         return e;
     }));
@@ -161,6 +161,14 @@ int launch_decode(const csv_plan* plan, const kv_pool* pool, int layer, const vo
     if (const char* e = getenv("CSV_X_DECODE_PF")) p.l2_prefetch = std::max(0, std::min(24, atoi(e)));   // experiment knob
     if (s.head_dim == 128) {
         if (plan->decode_warps == 2) return launch_decode_t<128, 4, 2>(plan, p, (cudaStream_t)stream);
+        int st = plan->decode_warps == kDecodeWarps128 ? 2 : 3;
+        if (const char* e = getenv("CSV_X_DECODE_STAGES")) st = atoi(e);   // experiment knobs
+#define CSV_TRY_SW(S, W) \
+        if (st == S && plan->decode_warps == W) return launch_decode_t<128, S, W>(plan, p, (cudaStream_t)stream);
+        CSV_TRY_SW(2, 8) CSV_TRY_SW(2, 7) CSV_TRY_SW(2, 6) CSV_TRY_SW(2, 5) CSV_TRY_SW(2, 4)
+        CSV_TRY_SW(3, 7) CSV_TRY_SW(3, 6) CSV_TRY_SW(3, 5) CSV_TRY_SW(3, 4)
+        CSV_TRY_SW(4, 6) CSV_TRY_SW(4, 5) CSV_TRY_SW(4, 4)
+#undef CSV_TRY_SW
         return launch_decode_t<128, 3, 8>(plan, p, (cudaStream_t)stream);
     }
     return launch_decode_t<64, 6, 8>(plan, p, (cudaStream_t)stream);

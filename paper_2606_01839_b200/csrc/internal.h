@@ -67,7 +67,8 @@ struct MergeGroup {
     int32_t pad;
 };
 
-constexpr int kDecodeWarps = 8;      // independent warp-workers per decode CTA
+constexpr int kDecodeWarps = 8;      // independent warp-workers per decode CTA (d = 64)
+constexpr int kDecodeWarps128 = 7;   // ... at d = 128, with 2-stage rings
 constexpr int kAppendTileRows = 64;  // stacked rows per append work item of the mma.sync kernel (4 warps x 16)
 constexpr int kAppendTileRowsTc2 = 256;  // ... of the two-tile tcgen05 kernel (two UMMA M = 128 tiles sharing K/V)
 constexpr int kAppendKvSplit = 8192; // default KV tokens per append partition
@@ -96,7 +97,7 @@ struct csv_plan {
     std::vector<MergeGroup> decode_groups;   // groups with count > 1 only
     int32_t n_decode_rows;
     int32_t decode_grid;                     // CTAs
-    int32_t decode_warps;                    // warp-workers per CTA (8; 2 = the slim kernel that runs beside the append CTAs)
+    int32_t decode_warps;                    // warp-workers per CTA (7 at d = 128, 8 at d = 64; others: experiment knobs)
     int32_t n_decode_partials;               // partial slots (non-direct items)
     std::vector<int32_t> zero_rows;          // q rows of decode conversations with kv_len = 0 (O = 0, LSE = -inf)
     // mixed step in one launch (tail_kernel): the decode rows cut again for tail_n_dec CTAs x 8 warp-workers

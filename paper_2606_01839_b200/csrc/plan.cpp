@@ -168,6 +168,11 @@ static void plan_tail(csv_plan* p) {
     if (const char* e = getenv("CSV_X_TAIL_SM_GBS")) sm_gbs = atof(e);         // experiment knobs
     if (const char* e = getenv("CSV_X_TAIL_SM_TFLOPS")) sm_tflops = atof(e);
     const double td = bytes / (sm_gbs * 1e9), ta = flops / (sm_tflops * 1e12);   // SM-seconds of each role
+    // The one launch pays when the decode rows are a sizeable part of the step (configs[2]: td / (td + ta) = 0.34, one call
+    // 4.53 ms against 4.73 for the two kernels back to back); with little decode work beside long chunks (configs[4]: 0.16)
+    // giving SMs to the decode role for the whole launch costs more than it hides (8-layer step 46.1 against 44.4 ms), and
+    // csv_tail_step keeps the two kernels.
+    if (td < 0.25 * (td + ta) && !getenv("CSV_X_TAIL_NDEC")) return;
     // A decode side that is too small costs more than one that is too large (SMs that finish their decode share take chunk
     // items, while a chunk-role SM can only take over a whole share), so the split leans 8 % towards decode.
     int k = (int)(1.08 * p->num_sms * td / (td + ta) + 0.5);
@@ -349,8 +354,15 @@ csv_plan* csv_plan_build_host(const csv_attn_shape* shape, const int32_t* h_q_le
     for (int b = 0; b < batch; ++b) p->q_start[(size_t)b + 1] = p->q_start[(size_t)b] + h_q_lens[b];
     p->total_q = (int32_t)total_q;
     p->d_ws = nullptr;
-    p->decode_warps = kDecodeWarps;
-    if (const char* e = getenv("CSV_X_DECODE_WARPS")) p->decode_warps = atoi(e) == 2 ? 2 : kDecodeWarps;   // experiment knob
+    // d = 128: 7 warp-workers x 2 ring stages per SM (112 KB in flight).  Measured against 8 x 3 (192 KB): configs[1] 184.8
+    // against 201.2 us, configs[2] 2.02 against 2.12 ms, configs[4] 1.25 against 1.31 ms per layer (6 x 2: 184.8 us / 2.02 /
+    // 1.23 ms): more bytes in flight than the latency needs only queue up in the memory system.
+    // 7 rather than 6 keeps configs[4] at >= 64 partitions per sequence (8 KV heads x 8.1 shares) without extra cuts.
+    p->decode_warps = shape->head_dim == 128 ? kDecodeWarps128 : kDecodeWarps;
+    if (const char* e = getenv("CSV_X_DECODE_WARPS")) {   // experiment knob
+        const int w = atoi(e);
+        p->decode_warps = (w == 2 || (w >= 4 && w <= 8)) ? w : kDecodeWarps;
+    }
     plan_decode(p);
     plan_append(p);
     plan_tail(p);
@@ -387,6 +399,8 @@ int csv_plan_info(const csv_plan_t* plan, int32_t* n_decode_items, int32_t* n_de
     if (decode_grid) *decode_grid = plan->decode_grid;
     return CSV_OK;
 }
+
+int32_t csv_plan_decode_workers(const csv_plan_t* plan) { return plan ? (int32_t)plan->worker_begin.size() - 1 : -1; }
 
 int csv_plan_tail_split(const csv_plan_t* plan, int32_t* n_decode_ctas, int32_t* n_decode_shares) {
     if (!plan) return CSV_E_INVAL;
