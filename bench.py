@@ -35,6 +35,7 @@ import concurrent.futures
 import hashlib
 import json
 import os
+import re
 import socket
 import subprocess
 import sys
@@ -53,8 +54,9 @@ NOMINAL_HBM_GBS = 8000.0        # north_star's "~8 TB/s"; targets (70 % / 80 %) 
 O_TOL, LSE_TOL = 1e-2, 1e-3     # north_star's gates; the sampled rows of the timed configuration are checked live
 TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r2_traffic.csv")
 CSRC = os.path.join(ROOT, "paper_2606_01839_b200", "csrc")
-KERNEL_SOURCE = {"decode_kernel": "decode_attn.cu", "append_tc2_kernel": "append_attn_tc2.cu", "pack_kernel": "handoff.cu",
-                 "unpack_kernel": "handoff.cu", "direct_kernel": "handoff.cu", "tail_kernel": "tail_fused.cu"}
+KERNEL_SOURCE = {"decode_kernel": "decode_attn.cu+decode_worker.cuh", "append_tc2_kernel": "append_attn_tc2.cu+append_tc2_body.cuh",
+                 "pack_kernel": "handoff.cu", "unpack_kernel": "handoff.cu", "direct_kernel": "handoff.cu",
+                 "tail_kernel": "tail_fused.cu+decode_worker.cuh+append_tc2_body.cuh"}   # files whose change voids a capture
 
 
 # ------------------------------------------------------------------------------------------------ peaks, clocks
@@ -157,9 +159,13 @@ def graph_of(fn):
         return None
 
 
-def sha256_of(path):
+def sha256_of(files):
+    """sha256 over the named csrc files ("a.cu+b.cuh"), in order; None if one is missing."""
     try:
-        return hashlib.sha256(open(path, "rb").read()).hexdigest()
+        h = hashlib.sha256()
+        for f in files.split("+"):
+            h.update(open(os.path.join(CSRC, f), "rb").read())
+        return h.hexdigest()
     except Exception:
         return None
 
@@ -178,7 +184,7 @@ def traffic_for(kernel, config):
             best = d
     if best is None:
         return None, "no capture for this (kernel, config)"
-    cur = sha256_of(os.path.join(CSRC, best["source_file"]))
+    cur = sha256_of(best["source_file"])
     if cur != best["source_sha256"]:
         return None, "capture of commit %s is older than %s: refused" % (best["commit"], best["source_file"])
     return float(best["dram_read_bytes"]) + float(best["dram_write_bytes"]), \
@@ -669,7 +675,7 @@ def ingest_ncu(args):
     mult = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
     rd, wr, n = 0.0, 0.0, 0
     for r in rows[2:]:
-        if args.kernel not in r[col["Kernel Name"]]:
+        if not re.search(r"(?<![A-Za-z_])" + re.escape(args.kernel) + r"(?![A-Za-z_])", r[col["Kernel Name"]]):
             continue
         rd += float(r[col["dram__bytes_read.sum"]].replace(",", "")) * mult[units[col["dram__bytes_read.sum"]]]
         wr += float(r[col["dram__bytes_write.sum"]].replace(",", "")) * mult[units[col["dram__bytes_write.sum"]]]
@@ -683,10 +689,10 @@ def ingest_ncu(args):
         if new:
             f.write("# dram__bytes_read.sum / dram__bytes_write.sum per launch (mean over the captured launches) of `ncu --set full` "
                     "captures; written by `python bench.py --ingest-ncu REP --kernel K --config C` (commands: profiles/r2_README.md).\n"
-                    "# bench.py reports a row as roofline.traffic only while sha256(csrc/source_file) still equals source_sha256.\n")
+                    "# bench.py reports a row as roofline.traffic only while sha256 over the csrc files named in source_file still equals source_sha256.\n")
             f.write("kernel,config,dram_read_bytes,dram_write_bytes,launches,commit,source_file,source_sha256,report\n")
         f.write("%s,%s,%.0f,%.0f,%d,%s,%s,%s,%s\n" % (args.kernel, args.config, rd / n, wr / n, n, commit, src,
-                                                    sha256_of(os.path.join(CSRC, src)), os.path.basename(args.ingest_ncu)))
+                                                    sha256_of(src), os.path.basename(args.ingest_ncu)))
     print("%s %s: read %.4f GB, write %.4f GB per launch (%d launches)" % (args.kernel, args.config, rd / n / 1e9, wr / n / 1e9, n))
 
 

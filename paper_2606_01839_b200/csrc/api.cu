@@ -312,7 +312,7 @@ int csv_tail_step(const csv_plan_t* plan, kv_pool_t* pool, int32_t layer, const 
     if (plan->append_items.empty())   // decode rows only: the KV write rides in the decode launch
         return launch_decode(plan, pool, layer, d_q, d_block_tables, max_blocks, d_out, d_lse, stream, d_k_new, d_v_new);
     kv_pool view = layer_view_of(pool, layer);
-    static const bool no_fuse = getenv("CSV_X_TAIL_NOFUSE") != nullptr;   // experiment knob: the three-launch route
+    static const bool no_fuse = getenv("CSV_TAIL_TWO_KERNELS") != nullptr;   // tuning override: always the two-kernel route
     const bool fuse = plan->tail_n_dec > 0 && !no_fuse;
     int r = CSV_OK;
     if (fuse && write_kv) r = launch_tail_zero_queue(plan, stream);

@@ -81,11 +81,6 @@ __device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gmem_src, u
                  : "memory");
 }
 
-// asks the L2 to fetch [gmem_src, gmem_src + bytes) from HBM; no shared memory, no completion to wait for
-__device__ __forceinline__ void l2_prefetch(const void* gmem_src, uint32_t bytes) {
-    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(gmem_src), "r"(bytes) : "memory");
-}
-
 // ---- tensor-core fragments (legacy warp-level path, SASS HMMA / LDSM) -----------------------
 __device__ __forceinline__ void ldsm_x4(uint32_t (&r)[4], uint32_t addr) {
     asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];"

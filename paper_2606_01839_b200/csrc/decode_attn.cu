@@ -11,8 +11,10 @@
 //    stream (plan.cpp).  No __syncthreads anywhere; a long conversation never holds a CTA.
 //  * Lane 0 feeds the ring with 1-D bulk copies (cp.async.bulk, SASS UBLKCP): one 4 KiB K
 //    tile and one 4 KiB V tile per block, each contiguous in HBM and already in the 128-byte
-//    XOR-swizzled image ldmatrix wants (pool layout, conserve_kv.h).  8 warps x 3 stages x
-//    8 KiB = 192 KiB in flight per SM, well past the ~45 KiB/SM Little's law asks for.
+//    XOR-swizzled image ldmatrix wants (pool layout, conserve_kv.h).  At d = 128: 7 warps x
+//    2 stages x 8 KiB = 112 KiB in flight per SM (Little's law asks for ~45 KiB/SM).  Round 1
+//    ran 8 x 3 = 192 KiB: measured slower by 4-8 % on every config: bytes
+//    in flight beyond what the latency needs only queue up in the memory system.
 //  * The G query heads of the group are the (zero-padded) M rows of mma.sync.m16n8k16: one
 //    K/V tile read serves all G heads.  CUDA-core FMAs would need 2*d*(G+1) lane-ops per
 //    512 B of KV, 68-99 % of the FP32 issue rate at G = 8; HMMA makes
@@ -75,7 +77,7 @@ __global__ void decode_zero_rows_kernel(const int32_t* __restrict__ rows, int ro
 }
 
 template <int D, int STAGES, int WARPS>
-__global__ void __launch_bounds__(WARPS * 32, WARPS >= 4 ? 1 : 512 / (WARPS * 32)) decode_kernel(const __grid_constant__ DecodeParams p) {
+__global__ void __launch_bounds__(WARPS * 32, 1) decode_kernel(const __grid_constant__ DecodeParams p) {
     constexpr int TB = 16 * D * 2;   // tile bytes
     extern __shared__ __align__(1024) uint8_t smem[];
     const int warp = threadIdx.x >> 5;
@@ -91,11 +93,7 @@ int launch_decode_t(const csv_plan* plan, const DecodeParams& p, cudaStream_t st
     const size_t smem = (size_t)WARPS * STAGES * 2 * TB + (size_t)WARPS * STAGES * 8;
     static PerDeviceOnce attr;
     CSV_CUDA_TRY(once_per_device(attr, [&] {
-        cudaError_t e = cudaFuncSetAttribute(decode_kernel<D, STAGES, WARPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        // the slim variant runs BESIDE the append CTA: the SM must be carved for both kernels' shared memory at once
-        if (e == cudaSuccess && WARPS < 4)
-            e = cudaFuncSetAttribute(decode_kernel<D, STAGES, WARPS>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
-        return e;
+        return cudaFuncSetAttribute(decode_kernel<D, STAGES, WARPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     }));
     CSV_CUDA_TRY(launch_pdl(decode_kernel<D, STAGES, WARPS>, dim3(plan->decode_grid), dim3(WARPS * 32), smem, stream, p));
     const int ng = (int)plan->decode_groups.size();
@@ -157,19 +155,9 @@ int launch_decode(const csv_plan* plan, const kv_pool* pool, int layer, const vo
     p.Hkv = plan->shape.num_kv_heads;
     p.G = p.Hq / p.Hkv;
     p.scale_log2 = (float)(1.4426950408889634 / sqrt((double)s.head_dim));
-    p.l2_prefetch = 0;
-    if (const char* e = getenv("CSV_X_DECODE_PF")) p.l2_prefetch = std::max(0, std::min(24, atoi(e)));   // experiment knob
     if (s.head_dim == 128) {
-        if (plan->decode_warps == 2) return launch_decode_t<128, 4, 2>(plan, p, (cudaStream_t)stream);
-        int st = plan->decode_warps == kDecodeWarps128 ? 2 : 3;
-        if (const char* e = getenv("CSV_X_DECODE_STAGES")) st = atoi(e);   // experiment knobs
-#define CSV_TRY_SW(S, W) \
-        if (st == S && plan->decode_warps == W) return launch_decode_t<128, S, W>(plan, p, (cudaStream_t)stream);
-        CSV_TRY_SW(2, 8) CSV_TRY_SW(2, 7) CSV_TRY_SW(2, 6) CSV_TRY_SW(2, 5) CSV_TRY_SW(2, 4)
-        CSV_TRY_SW(3, 7) CSV_TRY_SW(3, 6) CSV_TRY_SW(3, 5) CSV_TRY_SW(3, 4)
-        CSV_TRY_SW(4, 6) CSV_TRY_SW(4, 5) CSV_TRY_SW(4, 4)
-#undef CSV_TRY_SW
-        return launch_decode_t<128, 3, 8>(plan, p, (cudaStream_t)stream);
+        // 7 warp-workers x 2 ring stages (the measured sweep of workers x stages)
+        return launch_decode_t<128, 2, kDecodeWarps128>(plan, p, (cudaStream_t)stream);
     }
     return launch_decode_t<64, 6, 8>(plan, p, (cudaStream_t)stream);
 }

@@ -23,7 +23,6 @@ struct DecodeParams {
     uint8_t* pool_layer_w;  // same address as pool_layer, writable (fused step)
     int32_t max_blocks, Hq, Hkv, G;
     float scale_log2;
-    int32_t l2_prefetch;   // blocks ahead of the ring that lane 0 asks the L2 to fetch (0 = off)
 };
 
 // worker: index into p.worker_begin; ring: STAGES x (K tile + V tile) of this warp; bars: STAGES mbarriers of this warp.
@@ -205,19 +204,6 @@ __device__ __forceinline__ void decode_worker(const DecodeParams& p, const int w
                     mbar_expect_tx(&bars[stage], 2 * TB);
                     bulk_g2s(dst, src, TB, &bars[stage]);
                     bulk_g2s(dst + TB, src + kv_stride, TB, &bars[stage]);
-                }
-            }
-            if (p.l2_prefetch > 0) {
-                // the shared-memory ring covers the L2 -> SM latency only; the HBM -> L2 leg is started l2_prefetch blocks early
-                const int far = nxt + p.l2_prefetch;
-                if (far < nblk && (far >> 5) <= grp_cur + 1) {
-                    const int id = (far >> 5) == grp_cur ? __shfl_sync(0xffffffffu, ids_cur, far & 31)
-                                                         : __shfl_sync(0xffffffffu, ids_nxt, far & 31);
-                    if (lane == 0) {
-                        const uint8_t* src = head_base + (size_t)id * blk_stride;
-                        l2_prefetch(src, TB);
-                        l2_prefetch(src + kv_stride, TB);
-                    }
                 }
             }
             if (i == pf_at && has_next) {

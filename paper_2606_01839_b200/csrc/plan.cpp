@@ -135,10 +135,8 @@ static void plan_decode(csv_plan* p) {
     // CTAs: one per SM, fewer when there is under 4 blocks of work per warp
     const int WPC = p->decode_warps;   // warp-workers per CTA
     int64_t want = (units + (int64_t)WPC * 4 - 1) / ((int64_t)WPC * 4);
-    int64_t max_grid = p->num_sms;
-    if (const char* e = getenv("CSV_X_DECODE_MULT")) max_grid *= std::max(1, atoi(e));   // experiment knob: slim CTAs per SM
-    p->decode_grid = (int)std::max<int64_t>(1, std::min<int64_t>(max_grid, want));
-    if (const char* e = getenv("CSV_X_DECODE_GRID")) p->decode_grid = std::max(1, std::min(p->decode_grid, atoi(e)));   // experiment knob
+    p->decode_grid = (int)std::max<int64_t>(1, std::min<int64_t>(p->num_sms, want));
+    if (const char* e = getenv("CSV_DECODE_GRID")) p->decode_grid = std::max(1, std::min(p->decode_grid, atoi(e)));   // tuning override
     build_decode_list(p, units, (int64_t)p->decode_grid * WPC, part_blocks, p->decode_items, p->worker_begin, p->decode_groups,
                       p->n_decode_partials);
 }
@@ -164,15 +162,14 @@ static void plan_tail(csv_plan* p) {
         if (m > 1) flops += 4.0 * d * Hq * m * ((double)(p->kv_lens[b] - m) + (m + 1) / 2.0);
     }
     const double bytes = (double)units * 2.0 * csv_tile_bytes(d);
-    double sm_gbs = 75.0, sm_tflops = 7.4;     // one SM: decode role pulls ~75 GB/s, append role sustains 7.0-7.8 TFLOP/s
-    if (const char* e = getenv("CSV_X_TAIL_SM_GBS")) sm_gbs = atof(e);         // experiment knobs
-    if (const char* e = getenv("CSV_X_TAIL_SM_TFLOPS")) sm_tflops = atof(e);
+    const double sm_gbs = 75.0, sm_tflops = 7.4;   // one SM: decode role pulls ~75 GB/s, append role sustains 7.0-7.8 TFLOP/s
     const double td = bytes / (sm_gbs * 1e9), ta = flops / (sm_tflops * 1e12);   // SM-seconds of each role
     // The one launch pays when the decode rows are a sizeable part of the step (configs[2]: td / (td + ta) = 0.34, one call
     // 4.53 ms against 4.73 for the two kernels back to back); with little decode work beside long chunks (configs[4]: 0.16)
     // giving SMs to the decode role for the whole launch costs more than it hides (8-layer step 46.1 against 44.4 ms), and
     // csv_tail_step keeps the two kernels.
-    if (td < 0.25 * (td + ta) && !getenv("CSV_X_TAIL_NDEC")) return;
+    const char* force = getenv("CSV_TAIL_DECODE_CTAS");   // tuning override: the decode-role CTAs of the one launch
+    if (td < 0.25 * (td + ta) && !force) return;
     // A decode side that is too small costs more than one that is too large (SMs that finish their decode share take chunk
     // items, while a chunk-role SM can only take over a whole share), so the split leans 8 % towards decode.
     int k = (int)(1.08 * p->num_sms * td / (td + ta) + 0.5);
@@ -180,12 +177,11 @@ static void plan_tail(csv_plan* p) {
     k = std::max(1, std::min(k, std::min(p->num_sms - 1, (p->num_sms * 3) / 4)));
     const int64_t want = (units + 8 * 4 - 1) / (8 * 4);
     k = (int)std::min<int64_t>(k, std::max<int64_t>(1, want));
-    if (const char* e = getenv("CSV_X_TAIL_NDEC")) k = std::max(1, std::min(p->num_sms - 1, atoi(e)));
+    if (force) k = std::max(1, std::min(p->num_sms - 1, atoi(force)));
     p->tail_n_dec = k;
     // shares per decode-role SM (measured on configs[2] / [4]: 1 share 4.64 / 5.07 ms, 4 shares 4.98 / 5.26 ms: every share
     // ends with a CTA-wide barrier and restarts the rings)
-    int shares = 1;
-    if (const char* e = getenv("CSV_X_TAIL_SHARES")) shares = std::max(1, std::min(16, atoi(e)));
+    const int shares = 1;
     p->tail_n_shares = (int)std::max<int64_t>(1, std::min<int64_t>((int64_t)k * shares, want));
     const int part_blocks = std::max(1, p->max_partition_tokens / CSV_BLOCK_SIZE);
     build_decode_list(p, units, (int64_t)p->tail_n_shares * 8, part_blocks, p->tail_items, p->tail_worker_begin, p->tail_groups,
@@ -359,10 +355,6 @@ csv_plan* csv_plan_build_host(const csv_attn_shape* shape, const int32_t* h_q_le
     // 1.23 ms): more bytes in flight than the latency needs only queue up in the memory system.
     // 7 rather than 6 keeps configs[4] at >= 64 partitions per sequence (8 KV heads x 8.1 shares) without extra cuts.
     p->decode_warps = shape->head_dim == 128 ? kDecodeWarps128 : kDecodeWarps;
-    if (const char* e = getenv("CSV_X_DECODE_WARPS")) {   // experiment knob
-        const int w = atoi(e);
-        p->decode_warps = (w == 2 || (w >= 4 && w <= 8)) ? w : kDecodeWarps;
-    }
     plan_decode(p);
     plan_append(p);
     plan_tail(p);

@@ -31,15 +31,9 @@ constexpr uint32_t kTailDecBarOff = smem_bytes2(4);                       // aft
 constexpr uint32_t kTailSmem = kTailDecBarOff + 8 * kTailDecStages * 8 + 64;
 static_assert(8u * kTailDecStages * 2u * 4096u <= AppendTc2Smem<4>::kOffBar2, "decode rings must fit in front of the barrier block");
 
-__device__ __forceinline__ uint32_t sm_id() {
-    uint32_t r;
-    asm volatile("mov.u32 %0, %%smid;" : "=r"(r));
-    return r;
-}
-
 __global__ void __launch_bounds__(kT2Threads, 1) tail_kernel(const __grid_constant__ AppendTc2Params pa,
                                                              const __grid_constant__ DecodeParams pd, const int n_dec,
-                                                             const int n_shares, const int num_sms, const int spread) {
+                                                             const int n_shares) {
     extern __shared__ __align__(1024) uint8_t smem[];
     const uint32_t tmem = append_tc2_setup<4>(smem);
     const int warp = threadIdx.x >> 5;
@@ -64,10 +58,7 @@ __global__ void __launch_bounds__(kT2Threads, 1) tail_kernel(const __grid_consta
             fence_proxy_async();   // the rings go back to the bulk-copy (async) proxy of whoever uses them next
         }
     };
-    // n_dec of the num_sms SM ids, evenly spread (Bresenham), start in the decode role
-    const int sm = spread ? (int)(sm_id() % (uint32_t)num_sms) : (int)blockIdx.x;
-    const bool dec_first = spread ? ((sm + 1) * n_dec) / num_sms != (sm * n_dec) / num_sms : sm < n_dec;
-    if (dec_first) decode_shares();
+    if ((int)blockIdx.x < n_dec) decode_shares();   // the first n_dec CTAs start in the decode role
     // append items (sched[0] = next unclaimed item)
     __syncthreads();
     if (threadIdx.x == 0) *slot = atomicAdd(pa.sched, 1u);
@@ -126,7 +117,6 @@ int launch_tail_fused(const csv_plan* plan, const kv_pool* pool, int layer, cons
     pd.Hkv = pa.Hkv;
     pd.G = pa.G;
     pd.scale_log2 = scale_log2;
-    pd.l2_prefetch = 0;
     const int n_dec = plan->tail_n_dec, n_shares = plan->tail_n_shares, grid = plan->num_sms;
     // the work queues must start at zero whatever happened to an earlier launch on this plan; with pdl the caller has
     // enqueued launch_tail_zero_queue BEFORE the kernel this one is chained to (a memset between them would break the chain)
@@ -138,13 +128,10 @@ int launch_tail_fused(const csv_plan* plan, const kv_pool* pool, int layer, cons
     CSV_CUDA_TRY(once_per_device(attr, [] {
         return cudaFuncSetAttribute(tail_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTailSmem);
     }));
-    int spread = 0;
-    if (const char* e = getenv("CSV_X_TAIL_SPREAD")) spread = atoi(e);   // experiment knob
     if (pdl)
-        CSV_CUDA_TRY(launch_pdl(tail_kernel, dim3(grid), dim3(kT2Threads), kTailSmem, (cudaStream_t)stream, pa, pd, n_dec, n_shares,
-                                grid, spread));
+        CSV_CUDA_TRY(launch_pdl(tail_kernel, dim3(grid), dim3(kT2Threads), kTailSmem, (cudaStream_t)stream, pa, pd, n_dec, n_shares));
     else
-        tail_kernel<<<grid, kT2Threads, kTailSmem, (cudaStream_t)stream>>>(pa, pd, n_dec, n_shares, grid, spread);
+        tail_kernel<<<grid, kT2Threads, kTailSmem, (cudaStream_t)stream>>>(pa, pd, n_dec, n_shares);
     CSV_CUDA_TRY(cudaGetLastError());
     // two merges behind it: the decode groups of the tail share list, the append groups
     int rc = launch_decode_merge_128(plan, plan->lay.tail_groups, (int)plan->tail_groups.size(), out, lse, stream);
