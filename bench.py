@@ -775,7 +775,7 @@ def run_ours(args):
     fields, head, wl, L = leg_long_context(args, rank, world, ranks_on_dev, dist, agg_dev, pk, sampler)
 
     p2p = None
-    if world >= 2 and ndev >= 2:
+    if world >= 2 and (ndev >= 2 or args.p2p):
         # the paper's one exchange step, prefiller (rank 0) -> decoder (rank 1), over NVLink
         try:
             from paper_2606_01839_b200 import handoff_p2p
@@ -783,10 +783,9 @@ def run_ours(args):
             p2p = handoff_p2p.run(dist, rank, tokens=8192, layers=32, convs=4, iters=3)
         except Exception as e:
             p2p = {"error": repr(e)[:300]}
-        if isinstance(p2p, dict) and dist is not None:
-            box = [p2p if rank == 1 else None]
-            dist.broadcast_object_list(box, src=1)
-            p2p = box[0]
+        box = [p2p if rank == 1 else None]          # the decoder (rank 1) holds the record; every rank joins the broadcast
+        dist.broadcast_object_list(box, src=1)
+        p2p = box[0]
     if rank != 0:
         if sampler:
             sampler.stop()
@@ -905,6 +904,8 @@ def main():
     ap.add_argument("--no-extras", action="store_true")
     ap.add_argument("--no-graph", action="store_true")
     ap.add_argument("--layers", type=int, default=0, help="cap on the resident layers of configs[4] (default: all 8 that fit)")
+    ap.add_argument("--p2p", action="store_true", help="time the prefiller -> decoder handoff between ranks 0 and 1 even when "
+                    "they share one device (it always runs when two devices are visible)")
     ap.add_argument("--only", default=None)
     ap.add_argument("--ingest-ncu", default=None)
     ap.add_argument("--kernel", default=None)

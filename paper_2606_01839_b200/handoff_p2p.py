@@ -52,9 +52,9 @@ def run(dist, rank, tokens=8192, layers=32, convs=4, iters=3, prefiller=0, decod
       copy    kv_pack_batch into LOCAL staging, csv_ipc_copy (cudaMemcpyAsync, the copy engine) of each message into the
               decoder's staging, then the local kv_unpack_batch: SURVEY NEXT-1's cudaMemcpyPeerAsync comparison.
     Returns the record on the decoder rank, None elsewhere."""
+    grp = dist.new_group([prefiller, decoder]) if dist.get_world_size() > 2 else None   # collective: every rank calls it
     if rank not in (prefiller, decoder):
         return None
-    grp = dist.new_group([prefiller, decoder]) if dist.get_world_size() > 2 else None
     ngpu = torch.cuda.device_count()
     NL, Hkv, d = layers, 8, 128
     toks = [max(16, tokens - 37 * i) for i in range(convs)]        # ragged last blocks
