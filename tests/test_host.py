@@ -325,3 +325,21 @@ def test_handoff_direct_and_ipc_reject_bad_arguments_before_touching_cuda():
     assert L.csv_ipc_open(buf, 0, None) == B.CSV_E_INVAL
     assert L.csv_ipc_close(ctypes.c_void_p(k)) == B.CSV_E_INVAL                   # never opened
     assert pool.used_blocks == 0
+
+
+def test_committed_ncu_traffic_rows_belong_to_the_current_kernel_sources():
+    # bench.py reports roofline.traffic only from a capture taken on the kernel sources as they are now (sha256 recorded at
+    # ingest time in profiles/r2_traffic.csv).  A kernel edit without a fresh capture must show up here, not as a silent null.
+    import importlib.util
+    import os
+
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    spec = importlib.util.spec_from_file_location("bench_module", os.path.join(root, "bench.py"))
+    bench = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(bench)
+    want = [("decode_kernel", "configs[1]"), ("decode_kernel", "configs[2]"), ("decode_kernel", "configs[4]"),
+            ("append_tc2_kernel", "configs[2]"), ("append_tc2_kernel", "configs[4]"), ("tail_kernel", "configs[2]"),
+            ("pack_kernel", "configs[3]"), ("unpack_kernel", "configs[3]"), ("direct_kernel", "configs[3]")]
+    for kernel, config in want:
+        traffic, why = bench.traffic_for(kernel, config)
+        assert traffic is not None and traffic > 0, "%s on %s: %s" % (kernel, config, why)
