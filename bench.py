@@ -425,7 +425,11 @@ def leg_long_context_extras(wl, L, pk, iters=6):
             "one_call_vs_sum_of_parts": oc["median_ms"] / parts_ms,
             "hbm_bound_ms": L * (wl.decode_kv_bytes() + app.append_kv_bytes()) / pk["hbm"] / 1e6,
             "tensor_bound_ms": L * app.append_flops() / pk["bf16_sustained"] / 1e9,
-            "decode_role_ctas": mixed.plan.info().get("tail_n_dec")}
+            "decode_role_ctas": mixed.plan.info().get("tail_n_dec"),
+            "note": "sum_of_parts = each call timed alone, a few launches on a cool chip; the %d-layer graph runs ~45 ms at the "
+                    "1000 W cap (sw_power_cap), where the same calls are 10-13 %% slower whichever way they are launched "
+                    "(separate_calls_ms is the like-for-like figure); decode_role_ctas 0 = the plan kept the two-kernel route "
+                    "(decode is under a quarter of this step)" % L}
     del mixed
     return blocks, [step], app
 
