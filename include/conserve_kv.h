@@ -356,6 +356,41 @@ int paged_decode_attn(const csv_plan_t* plan, const kv_pool_t* pool, int32_t lay
                       const int32_t* d_block_tables, int32_t max_blocks, void* d_out, float* d_lse,
                       void* stream);
 
+/* paged_decode_attn for callers that cannot allocate device memory and have no workspace to pass.
+ *
+ * Two kinds of caller are meant.  (1) A decoder that gave all of its HBM to the KV pool at start-up
+ * (§5.1: a decoder's memory is its ~300k-token KV budget): later cudaMalloc calls may simply fail.
+ * (2) A step that runs inside an engine which owns the device allocator, where cudaMalloc / cudaFree are off
+ * limits because they can fail mid-request and stall every stream of the device while they run.
+ * Every other attention call here needs a caller-owned plan workspace; this one needs only inputs and outputs.
+ *
+ * It builds the step's split-K plan on the host (host heap only), puts the work lists and the fp32 partials in
+ * a fixed CSV_STATIC_SCRATCH_BYTES array that is part of the library's device image, and runs the same kernels
+ * as paged_decode_attn: every conversation b in [0, batch) is one decode row (q_len 1) over h_kv_lens[b] cached
+ * tokens, with d_q / d_out [batch][Hq][d] bf16, d_lse [batch][Hq] fp32, d_block_tables [batch][max_blocks];
+ * results, kv_len = 0 behaviour and precision are those of paged_decode_attn on the same lengths and
+ * max_partition_tokens (bit-identical: same plan, same kernels).  No cudaMalloc, cudaFree, pinned-host or other
+ * allocating CUDA call is made; the call enqueues on `stream` and returns without synchronising.
+ *
+ * Limits and sharing, all of which the caller has to know:
+ *  - The array costs CSV_STATIC_SCRATCH_BYTES (8 MiB) on EVERY GPU on which this library's code is loaded, for
+ *    the life of the process, used or not.
+ *  - A step whose plan needs more than that returns CSV_E_NOMEM and launches nothing (csv_plan_workspace_bytes
+ *    with q_lens all 1 tells the need in advance; BASELINE.json's five configs need 0.03 - 4.9 MB).
+ *  - One array per GPU, shared by every call: a call overwrites what the previous one left (it re-uploads its
+ *    lists, queue words included, and only reads partial slots it has written itself, so nothing stale is ever
+ *    consumed), and calls that overlap on one GPU (two streams, two threads) corrupt each other.  Keep them on
+ *    one stream or order them with events.
+ *  - The first call on each device looks up the array's device address (cudaGetSymbolAddress, with that device
+ *    current).  Make that first call before starting any stream capture on the device.
+ * Errors: CSV_E_INVAL (bad pointer / alignment / shape / layer, negative length, max_blocks too small),
+ * CSV_E_NOMEM (over the limit above), CSV_E_CUDA. */
+#define CSV_STATIC_SCRATCH_BYTES (8u << 20)
+int paged_decode_attn_static(const kv_pool_t* pool, int32_t layer, const csv_attn_shape* shape, int32_t batch,
+                             const int32_t* h_kv_lens, int32_t max_partition_tokens, const void* d_q,
+                             const int32_t* d_block_tables, int32_t max_blocks, void* d_out, float* d_lse,
+                             void* stream);
+
 /* Fused decode tail step (§2.1: decode "generates each subsequent token by reading the
  * full KV cache and appending one new entry"): kv_append_tokens for the q_len = 1 rows of ONE layer
  * and paged_decode_attn in a single launch.  d_k_new, d_v_new: this layer's new-token K / V,

@@ -24,6 +24,7 @@ SYMBOLS = [
     "csv_plan_create", "csv_plan_destroy", "csv_plan_info", "csv_plan_tail_split", "csv_plan_decode_workers", "csv_plan_total_q", "csv_plan_decode_items",
     "csv_plan_append_items", "paged_decode_attn", "paged_decode_step", "append_prefill_attn", "csv_tail_step_host_workspace_bytes",
     "csv_tail_step_host", "kv_handoff_direct", "kv_handoff_direct_batch", "csv_ipc_export", "csv_ipc_open", "csv_ipc_close", "csv_ipc_copy", "csv_tail_step",
+    "paged_decode_attn_static",
 ]
 IPC_HANDLE_BYTES = 64
 
@@ -96,6 +97,7 @@ def lib():
             "csv_plan_decode_items": (i32, [vp, pi32, i32, pi32, i32]),
             "csv_plan_append_items": (i32, [vp, pi32, i32]),
             "paged_decode_attn": (ctypes.c_int, [vp, vp, i32, vp, vp, i32, vp, vp, vp]),
+            "paged_decode_attn_static": (ctypes.c_int, [vp, i32, pshape, i32, pi32, i32, vp, vp, i32, vp, vp, vp]),
             "append_prefill_attn": (ctypes.c_int, [vp, vp, i32, vp, vp, i32, vp, vp, vp]),
             "paged_decode_step": (ctypes.c_int, [vp, vp, i32, vp, vp, vp, vp, i32, vp, vp, vp]),
             "csv_tail_step": (ctypes.c_int, [vp, vp, i32, vp, vp, vp, vp, i32, vp, vp, vp]),
@@ -378,6 +380,27 @@ csv_plan_create = Plan
 def paged_decode_attn(plan, pool, layer, d_q, d_block_tables, max_blocks, d_out, d_lse, stream=None):
     _check("paged_decode_attn", lib().paged_decode_attn(plan.handle, pool.handle, layer, _ptr(d_q), _ptr(d_block_tables),
                                                         max_blocks, _ptr(d_out), _ptr(d_lse), _stream(stream)))
+
+
+STATIC_SCRATCH_BYTES = 8 << 20   # CSV_STATIC_SCRATCH_BYTES of conserve_kv.h
+
+
+def paged_decode_attn_static(pool, layer, shape, kv_lens, d_q, d_block_tables, max_blocks, d_out, d_lse,
+                             max_partition_tokens=0, stream=None):
+    """paged_decode_attn without a Plan or a workspace tensor, for callers that may not allocate device memory (all HBM
+    already belongs to the KV pool, or the surrounding engine forbids cudaMalloc inside a step).  One decode row per entry
+    of kv_lens.  The scratch is a fixed 8 MiB array inside the library, one per GPU, shared by every call: keep calls on
+    one stream.  A step that needs more raises CsvError(CSV_E_NOMEM); make the first call on a device before any stream
+    capture (it looks the array's address up).  See conserve_kv.h."""
+    k, pk = _i32(kv_lens)
+    rc = lib().paged_decode_attn_static(pool.handle, layer, ctypes.byref(shape), len(k), pk, max_partition_tokens, _ptr(d_q),
+                                        _ptr(d_block_tables), max_blocks, _ptr(d_out), _ptr(d_lse), _stream(stream))
+    if rc == CSV_E_NOMEM:
+        err = CsvError("paged_decode_attn_static", rc)
+        err.args = ("%s: this step's plan needs more than the library's fixed %d-byte scratch array; use paged_decode_attn "
+                    "with a caller-owned workspace" % (err.args[0], STATIC_SCRATCH_BYTES),)
+        raise err
+    _check("paged_decode_attn_static", rc)
 
 
 def paged_decode_step(plan, pool, layer, d_q, d_k_new, d_v_new, d_block_tables, max_blocks, d_out, d_lse, stream=None):

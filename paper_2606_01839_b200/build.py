@@ -16,7 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libconserve_kv.so")
 OBJDIR = os.path.join(HERE, "build")
-SOURCES = ["pool.cpp", "plan.cpp", "api.cu", "handoff.cu", "decode_attn.cu", "append_attn.cu", "append_attn_tc2.cu", "tail_fused.cu"]
+SOURCES = ["pool.cpp", "plan.cpp", "api.cu", "handoff.cu", "decode_attn.cu", "append_attn.cu", "append_attn_tc2.cu", "tail_fused.cu", "noalloc.cu"]
 HEADERS = ["internal.h", "common.cuh", "tc5.cuh", "decode_worker.cuh", "append_tc2_body.cuh", os.path.join("..", "..", "include", "conserve_kv.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC",
