@@ -72,6 +72,18 @@ def handoff_ticket(pool, tokens, token_offset=0, ids=None, export=None, decoder=
             "handle": None if export is None else bytes(export[0]), "offset": 0 if export is None else int(export[1])}
 
 
+def validate_ticket(ticket):
+    """Prefiller side, before any launch that uses a ticket's ids.  The ids came over a channel and the kernels do not
+    range-check them (conserve_kv.h): one bad id would be a silent out-of-bounds write into another process's allocation.
+    Checks the table against the ticket's own shape; PeerPools.get bounds that shape by the mapped allocation."""
+    ids, nb = ticket["ids"], int(ticket["shape"][1])
+    need = (ticket["token_offset"] + ticket["tokens"] + 15) // 16
+    if ticket["tokens"] <= 0 or ticket["token_offset"] < 0 or len(ids) < need:
+        raise ValueError("ticket: table shorter than ceil((offset + tokens) / 16)")
+    if any((not isinstance(i, int)) or i < 0 or i >= nb for i in ids) or len(set(ids)) != len(ids):
+        raise ValueError("ticket: block ids must be unique and inside [0, num_blocks)")
+
+
 def send_ticket(dist, ticket, dst):
     dist.send_object_list([ticket], dst=dst)
 
@@ -115,14 +127,7 @@ class PeerPools:
         from . import binding as B
 
         pool = self.get(ticket, local_pool)
-        # The ids came over a channel and the kernel does not range-check them (conserve_kv.h): one bad id would be a
-        # silent out-of-bounds write into another process's allocation.  Validate on the host before launching.
-        ids, nb = ticket["ids"], ticket["shape"][1]
-        need = (ticket["token_offset"] + ticket["tokens"] + 15) // 16
-        if ticket["tokens"] <= 0 or ticket["token_offset"] < 0 or len(ids) < need:
-            raise ValueError("ticket: table shorter than ceil((offset + tokens) / 16)")
-        if any((not isinstance(i, int)) or i < 0 or i >= nb for i in ids) or len(set(ids)) != len(ids):
-            raise ValueError("ticket: block ids must be unique and inside [0, num_blocks)")
+        validate_ticket(ticket)
         if d_ids is None:
             d_ids = torch.tensor(ticket["ids"], dtype=torch.int32, device="cuda")
         B.kv_handoff_direct(pool, d_k, d_v, ticket["tokens"], ticket["token_offset"], d_ids, len(ticket["ids"]), stream)
