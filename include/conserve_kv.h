@@ -245,6 +245,10 @@ int kv_handoff_direct_batch(kv_pool_t* dst, int32_t n, const void* const* h_d_k,
  *   lazily when it lives on another GPU) and returns base + offset.
  *   Opens of the same allocation are counted (several exported pointers may
  *   share one allocation); the mapping goes away with the last close.
+ * csv_ipc_mapped_bytes: d_ptr is what csv_ipc_open returned; writes how many bytes of the mapped allocation lie
+ *   at and after d_ptr (0 if the sender's offset points past its end).  The opener uses it to refuse a pool
+ *   descriptor that claims more memory than the sender really shared, before wrapping the pointer in a kv_pool_t:
+ *   shape and offset arrive in the same untrusted message as the handle.
  * csv_ipc_close: d_ptr is what csv_ipc_open returned (one close per open).
  * csv_ipc_copy: copy-engine transfer (cudaMemcpyAsync, device to device) of
  *   `bytes` bytes between two device pointers of which either may be a
@@ -256,6 +260,7 @@ int kv_handoff_direct_batch(kv_pool_t* dst, int32_t n, const void* const* h_d_k,
 #define CSV_IPC_HANDLE_BYTES 64
 int csv_ipc_export(const void* d_ptr, void* out_handle, uint64_t* out_offset);
 int csv_ipc_open(const void* handle, uint64_t offset, void** out_d_ptr);
+int csv_ipc_mapped_bytes(const void* d_ptr, size_t* out_bytes);
 int csv_ipc_close(void* d_ptr);
 int csv_ipc_copy(void* d_dst, const void* d_src, size_t bytes, void* stream);
 
@@ -278,12 +283,28 @@ int kv_append_tokens(kv_pool_t* dst, const csv_plan_t* plan, const void* d_k_new
  * decode row, q_len m > 1 = appended chunk with prefix P = kv_len - m.
  *
  * Split-K: the flattened (conversation, block) stream of the q_len = 1 rows is
- * cut into one contiguous share per warp-worker (8 per CTA), and each share into
+ * cut into one contiguous share per warp-worker (7 per CTA at head_dim 128, 8 at 64), and each share into
  * partitions that never cross a (conversation, KV head) boundary and, if
  * max_partition_tokens > 0 (a multiple of 16), hold at most that many tokens
  * (0 = no extra cut).  The schedule depends only on the lengths, so
  * results are bit-identical under any block permutation and from run to run.
  * ---------------------------------------------------------------------- */
+
+/* Tuning overrides (measurement aids; the defaults are what the bench times).  One process-wide table, read when a
+ * plan is BUILT (csv_plan_workspace_bytes, csv_plan_create, the *_host calls) and recorded in it: later changes do not
+ * affect existing plans, and a workspace size always matches a plan built under the same settings.  value 0 = default.
+ *   CSV_TUNE_DECODE_GRID        cap on the CTAs of the decode launch (default: one per SM)
+ *   CSV_TUNE_TAIL_DECODE_CTAS   decode-role CTAs of a mixed step's one launch, also where the planner would have kept
+ *                               the two kernels (default: chosen from the two roles' work, conserve_kv.h csv_tail_step)
+ *   CSV_TUNE_TAIL_TWO_KERNELS   non-zero: csv_tail_step never uses the one-launch route for plans built from now on
+ * At first use each knob is initialised from the environment variable of the same name without "TUNE_"
+ * (CSV_DECODE_GRID, CSV_TAIL_DECODE_CTAS: a positive decimal integer, anything else is ignored; CSV_TAIL_TWO_KERNELS:
+ * any value other than 0).  Not thread-safe against concurrent plan builds.  csv_tuning_get returns -1 for a bad knob. */
+#define CSV_TUNE_DECODE_GRID       0
+#define CSV_TUNE_TAIL_DECODE_CTAS  1
+#define CSV_TUNE_TAIL_TWO_KERNELS  2
+int csv_tuning_set(int32_t knob, int32_t value);
+int32_t csv_tuning_get(int32_t knob);
 
 /* Device workspace the plan needs (partials, work lists), for these lengths. */
 size_t csv_plan_workspace_bytes(const csv_attn_shape* shape, const int32_t* h_q_lens,
@@ -324,7 +345,7 @@ int32_t csv_plan_total_q(const csv_plan_t* plan);
 /* Copies the decode work list for inspection (host tests): item i is 8 int32
  * {conv, kv_head, blk_begin, blk_end, kv_len, partial, direct, q_row} at h_out[8*i];
  * h_worker_begin[w] .. h_worker_begin[w+1] are the items of warp-worker w
- * (decode_grid * 8 workers).  Either output may be NULL.  Returns the item count. */
+ * (csv_plan_decode_workers(plan) of them).  Either output may be NULL.  Returns the item count. */
 int32_t csv_plan_decode_items(const csv_plan_t* plan, int32_t* h_out, int32_t max_items,
                               int32_t* h_worker_begin, int32_t max_workers_plus_1);
 /* Same for the append work list: item i is 12 int32 {conv, kv_head, row_begin,
@@ -453,8 +474,13 @@ int csv_tail_step(const csv_plan_t* plan, kv_pool_t* pool, int32_t layer, const 
  * they fly (lengths are per step, not per layer), runs csv_tail_step on every
  * layer, copies O and LSE back and synchronises `stream`.  Host buffers should
  * be pinned.  d_workspace: >= csv_tail_step_host_workspace_bytes(...), 128-byte
- * aligned.  Errors as csv_plan_create / csv_tail_step; nothing is launched on
- * CSV_E_INVAL / CSV_E_NOMEM.
+ * aligned.  Errors as csv_plan_create / csv_tail_step.  Every CSV_E_INVAL case
+ * (pointers, shape, lengths, partition size) and a workspace smaller than the
+ * buffers is refused before anything is enqueued.  A workspace that holds the
+ * buffers but not the plan (CSV_E_NOMEM) or a CUDA failure part-way is only found
+ * after the input copies were enqueued: the call then synchronises `stream`
+ * before returning the error, so no DMA from the host buffers is left in flight
+ * (the pool may hold some layers' new rows; outputs are unspecified).
  * ---------------------------------------------------------------------- */
 size_t csv_tail_step_host_workspace_bytes(const csv_attn_shape* shape, const int32_t* h_q_lens, const int32_t* h_kv_lens,
                                           int32_t batch, int32_t max_blocks, int32_t n_layers,

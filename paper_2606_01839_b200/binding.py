@@ -24,7 +24,7 @@ SYMBOLS = [
     "csv_plan_create", "csv_plan_destroy", "csv_plan_info", "csv_plan_tail_split", "csv_plan_decode_workers", "csv_plan_total_q", "csv_plan_decode_items",
     "csv_plan_append_items", "paged_decode_attn", "paged_decode_step", "append_prefill_attn", "csv_tail_step_host_workspace_bytes",
     "csv_tail_step_host", "kv_handoff_direct", "kv_handoff_direct_batch", "csv_ipc_export", "csv_ipc_open", "csv_ipc_close", "csv_ipc_copy", "csv_tail_step",
-    "paged_decode_attn_static",
+    "paged_decode_attn_static", "csv_ipc_mapped_bytes", "csv_tuning_set", "csv_tuning_get",
 ]
 IPC_HANDLE_BYTES = 64
 
@@ -86,7 +86,10 @@ def lib():
             "csv_ipc_export": (ctypes.c_int, [vp, vp, ctypes.POINTER(ctypes.c_uint64)]),
             "csv_ipc_open": (ctypes.c_int, [vp, ctypes.c_uint64, pvp]),
             "csv_ipc_close": (ctypes.c_int, [vp]),
+            "csv_ipc_mapped_bytes": (ctypes.c_int, [vp, ctypes.POINTER(sz)]),
             "csv_ipc_copy": (ctypes.c_int, [vp, vp, sz, vp]),
+            "csv_tuning_set": (ctypes.c_int, [i32, i32]),
+            "csv_tuning_get": (i32, [i32]),
             "csv_plan_workspace_bytes": (sz, [pshape, pi32, pi32, i32, i32]),
             "csv_plan_create": (ctypes.c_int, [pshape, pi32, pi32, i32, i32, vp, sz, vp, pvp]),
             "csv_plan_destroy": (ctypes.c_int, [vp]),
@@ -301,6 +304,13 @@ def csv_ipc_open(handle, offset):
     return int(out.value)
 
 
+def csv_ipc_mapped_bytes(ptr):
+    """Bytes of the mapped allocation at and after a pointer csv_ipc_open returned."""
+    out = ctypes.c_size_t()
+    _check("csv_ipc_mapped_bytes", lib().csv_ipc_mapped_bytes(ctypes.c_void_p(ptr), ctypes.byref(out)))
+    return int(out.value)
+
+
 def csv_ipc_close(ptr):
     _check("csv_ipc_close", lib().csv_ipc_close(ctypes.c_void_p(ptr)))
 
@@ -308,6 +318,18 @@ def csv_ipc_close(ptr):
 def csv_ipc_copy(dst, src, nbytes, stream=None):
     """Copy-engine transfer between device buffers (torch tensors or raw pointers, e.g. a csv_ipc_open mapping)."""
     _check("csv_ipc_copy", lib().csv_ipc_copy(_ptr(dst), _ptr(src), int(nbytes), _stream(stream)))
+
+
+TUNE_DECODE_GRID, TUNE_TAIL_DECODE_CTAS, TUNE_TAIL_TWO_KERNELS = 0, 1, 2
+
+
+def csv_tuning_set(knob, value):
+    """Process-wide tuning override (0 = default); read when a plan is built and recorded in it (conserve_kv.h)."""
+    _check("csv_tuning_set", lib().csv_tuning_set(knob, value))
+
+
+def csv_tuning_get(knob):
+    return int(lib().csv_tuning_get(knob))
 
 
 def csv_plan_workspace_bytes(shape, q_lens, kv_lens, max_partition_tokens=0):

@@ -203,6 +203,24 @@ int csv_ipc_close(void* d_ptr) {
     return CSV_E_INVAL;
 }
 
+int csv_ipc_mapped_bytes(const void* d_ptr, size_t* out_bytes) {
+    if (!d_ptr || !out_bytes) return CSV_E_INVAL;
+    for (const ipc_region& r : g_ipc)
+        for (void* u : r.users) {
+            if (u != d_ptr) continue;
+            cu_get_range_fn get_range = driver_get_range();
+            if (!get_range) return csv_set_cuda_error((int)cudaErrorNotSupported);
+            unsigned long long base = 0;
+            size_t size = 0;
+            if (get_range(&base, &size, (unsigned long long)(uintptr_t)r.base) != 0)
+                return csv_set_cuda_error((int)cudaErrorInvalidValue);
+            const uintptr_t end = (uintptr_t)base + size;
+            *out_bytes = (uintptr_t)d_ptr < end ? (size_t)(end - (uintptr_t)d_ptr) : 0;   // an offset past the end leaves nothing
+            return CSV_OK;
+        }
+    return CSV_E_INVAL;
+}
+
 int csv_ipc_copy(void* d_dst, const void* d_src, size_t bytes, void* stream) {
     if (!d_dst || !d_src) return CSV_E_INVAL;
     if (bytes == 0) return CSV_OK;
@@ -312,8 +330,7 @@ int csv_tail_step(const csv_plan_t* plan, kv_pool_t* pool, int32_t layer, const 
     if (plan->append_items.empty())   // decode rows only: the KV write rides in the decode launch
         return launch_decode(plan, pool, layer, d_q, d_block_tables, max_blocks, d_out, d_lse, stream, d_k_new, d_v_new);
     kv_pool view = layer_view_of(pool, layer);
-    static const bool no_fuse = getenv("CSV_TAIL_TWO_KERNELS") != nullptr;   // tuning override: always the two-kernel route
-    const bool fuse = plan->tail_n_dec > 0 && !no_fuse;
+    const bool fuse = plan->tail_n_dec > 0 && !plan->tail_two_kernels;   // tuning override recorded in the plan (csv_tuning_set)
     int r = CSV_OK;
     if (fuse && write_kv) r = launch_tail_zero_queue(plan, stream);
     if (r == CSV_OK && write_kv) r = launch_append_tokens(&view, plan, d_k_new, d_v_new, d_block_tables, max_blocks, stream);
@@ -386,6 +403,17 @@ int csv_tail_step_host(kv_pool_t* pool, int32_t layer_begin, int32_t n_layers, c
     if (shape->num_q_heads <= 0 || shape->num_q_heads % shape->num_kv_heads != 0) return CSV_E_INVAL;
     const int64_t rows = host_step_rows(h_q_lens, batch);   // per layer
     if (rows <= 0 || rows * n_layers > INT32_MAX) return CSV_E_INVAL;
+    // Everything csv_plan_build_host would refuse is refused HERE, before the first copy is enqueued: a CSV_E_INVAL must
+    // not leave DMA from the caller's host buffers in flight (the plan itself is still built under the copies, below).
+    {
+        const int g = shape->num_q_heads / shape->num_kv_heads;
+        if (g != 1 && g != 2 && g != 4 && g != 8) return CSV_E_INVAL;
+        if (max_partition_tokens < 0 || max_partition_tokens % CSV_BLOCK_SIZE != 0) return CSV_E_INVAL;
+        for (int b = 0; b < batch; ++b) {
+            const int32_t q = h_q_lens ? h_q_lens[b] : 1, kv = h_kv_lens[b];
+            if (kv < 0 || q < 0 || (q > kv && !(q == 1 && kv == 0))) return CSV_E_INVAL;
+        }
+    }
     // The plan's size is not known before it is built, so the fixed-size buffers sit in front of it: their copies
     // are enqueued first and fly while the host plans.
     const size_t q_layer = (size_t)rows * shape->num_q_heads * shape->head_dim * 2;
@@ -400,8 +428,10 @@ int csv_tail_step_host(kv_pool_t* pool, int32_t layer_begin, int32_t n_layers, c
         (e = cudaMemcpyAsync(ws + L.k, h_k_new, k_layer * n_layers, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
         (e = cudaMemcpyAsync(ws + L.v, h_v_new, k_layer * n_layers, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
         (e = cudaMemcpyAsync(ws + L.tables, h_block_tables, (size_t)batch * max_blocks * 4, cudaMemcpyHostToDevice, st)) !=
-            cudaSuccess)
+            cudaSuccess) {
+        (void)cudaStreamSynchronize(st);   // some copies may be in flight: the caller's buffers are free again on return
         return csv_set_cuda_error((int)e);
+    }
     // One plan serves every layer of the step (lengths are per step, not per layer).  It is built here, while the copies
     // above are in flight: measured on configs[1], keeping the previous step's plan alive and extending it (no planning,
     // pinned plan image) did not shorten the call (0.289 against 0.282 ms): the host work is hidden under the DMA.
@@ -409,7 +439,10 @@ int csv_tail_step_host(kv_pool_t* pool, int32_t layer_begin, int32_t n_layers, c
     if (!h_q_lens) ones.assign((size_t)batch, 1);
     int err;
     csv_plan_t* plan = csv_plan_build_host(shape, h_q_lens ? h_q_lens : ones.data(), h_kv_lens, batch, max_partition_tokens, &err);
-    if (!plan) return err;
+    if (!plan) {
+        (void)cudaStreamSynchronize(st);   // (only CSV_E_NOMEM of the host heap can get here: lengths were checked above)
+        return err;
+    }
     int rc = ws_bytes - L.plan < plan->lay.total ? CSV_E_NOMEM : plan_attach(plan, ws + L.plan, ws_bytes - L.plan, stream);
     for (int l = 0; rc == CSV_OK && l < n_layers; ++l)   // KV write of every new row + decode rows + appended chunks
         rc = csv_tail_step(plan, pool, layer_begin + l, ws + L.q + l * q_layer, ws + L.k + l * k_layer, ws + L.v + l * k_layer,
@@ -420,6 +453,10 @@ int csv_tail_step_host(kv_pool_t* pool, int32_t layer_begin, int32_t n_layers, c
             (e = cudaMemcpyAsync(h_lse, ws + L.lse, lse_layer * n_layers, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
             (e = cudaStreamSynchronize(st)) != cudaSuccess)
             rc = csv_set_cuda_error((int)e);
+    } else {
+        // Workspace too small for the plan, or a launch failed part-way: the input copies (and perhaps some layers' work)
+        // are enqueued.  Drain the stream so that nothing reads the caller's host buffers after the error is returned.
+        (void)cudaStreamSynchronize(st);
     }
     csv_plan_destroy(plan);
     return rc;

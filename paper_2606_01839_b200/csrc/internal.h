@@ -79,7 +79,7 @@ struct PlanLayout {   // byte offsets into the caller's workspace (all 128-byte 
     size_t tail_items, tail_worker_begin, tail_groups;   // the decode share list of tail_kernel's decode-role CTAs (mixed steps)
     size_t zero_rows;   // int32 rows of d_out / d_lse whose conversation has q_len = 1 and an empty cache
     size_t conv_meta;   // int32 [q_start[batch+1] | kv_len[batch] | q_len[batch]]
-    size_t append_sched;   // uint32 [next item, CTAs done]: the append kernel's work queue, zero between launches
+    size_t append_sched;   // uint32 [0] next append item, [1] CTAs done, [2] next decode share (tail_kernel): zeroed by a cudaMemsetAsync before every launch
     size_t total;
 };
 
@@ -103,6 +103,7 @@ struct csv_plan {
     // mixed step in one launch (tail_kernel): the decode rows cut again for tail_n_dec CTAs x 8 warp-workers
     int32_t tail_n_dec;                      // SMs that start in the decode role (0 = no fused launch for this plan)
     int32_t tail_n_shares;                   // decode shares of 8 warp-workers each (a queue: any CTA may take one)
+    int32_t tail_two_kernels;                // CSV_TUNE_TAIL_TWO_KERNELS in force when the plan was built: csv_tail_step keeps decode + append apart
     std::vector<DecodeItem> tail_items;
     std::vector<int32_t> tail_worker_begin;
     std::vector<MergeGroup> tail_groups;
@@ -142,6 +143,12 @@ int launch_tail_fused(const csv_plan* plan, const kv_pool* pool, int layer, cons
                       int max_blocks, void* out, float* lse, void* stream, bool pdl);
 int launch_append_attn_tc2(const csv_plan* plan, const kv_pool* pool, int layer, const void* q, const int32_t* tables,
                            int max_blocks, void* out, float* lse, void* stream);
+// Tuning knobs (conserve_kv.h csv_tuning_set): one process-wide table, initialised once from the environment; every plan
+// records what it was built with, so a plan and its workspace size cannot disagree unless the caller changes a knob between.
+struct CsvTuning {
+    int32_t v[3];   // indexed by CSV_TUNE_*; 0 = library default
+};
+CsvTuning& csv_tuning();
 int csv_query_num_sms();   // SM count of the current device, 148 if none is usable
 csv_plan* csv_plan_build_host(const csv_attn_shape* shape, const int32_t* h_q_lens, const int32_t* h_kv_lens,
                               int32_t batch, int32_t max_partition_tokens, int* err);

@@ -22,6 +22,23 @@
 
 static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
+// A knob from the environment: a positive decimal integer, or (two-kernel switch only) any non-empty value = 1.
+// Anything else is ignored rather than guessed at (atoi of garbage used to give a one-CTA grid).
+static int32_t env_knob(const char* name, bool flag) {
+    const char* e = getenv(name);
+    if (!e || !*e) return 0;
+    char* end = nullptr;
+    const long v = strtol(e, &end, 10);
+    if (end != e && *end == 0 && v > 0 && v <= (1 << 20)) return (int32_t)v;
+    return (flag && !(end != e && *end == 0)) ? 1 : 0;   // flag: "yes", "on", ... count as set; "0" does not
+}
+
+CsvTuning& csv_tuning() {
+    static CsvTuning t = {{env_knob("CSV_DECODE_GRID", false), env_knob("CSV_TAIL_DECODE_CTAS", false),
+                           env_knob("CSV_TAIL_TWO_KERNELS", true)}};
+    return t;
+}
+
 static bool attn_shape_ok(const csv_attn_shape* s) {
     if (!s) return false;
     if (s->block_size != CSV_BLOCK_SIZE) return false;
@@ -136,7 +153,7 @@ static void plan_decode(csv_plan* p) {
     const int WPC = p->decode_warps;   // warp-workers per CTA
     int64_t want = (units + (int64_t)WPC * 4 - 1) / ((int64_t)WPC * 4);
     p->decode_grid = (int)std::max<int64_t>(1, std::min<int64_t>(p->num_sms, want));
-    if (const char* e = getenv("CSV_DECODE_GRID")) p->decode_grid = std::max(1, std::min(p->decode_grid, atoi(e)));   // tuning override
+    if (const int32_t cap = csv_tuning().v[CSV_TUNE_DECODE_GRID]) p->decode_grid = std::max(1, std::min(p->decode_grid, cap));   // tuning override
     build_decode_list(p, units, (int64_t)p->decode_grid * WPC, part_blocks, p->decode_items, p->worker_begin, p->decode_groups,
                       p->n_decode_partials);
 }
@@ -168,7 +185,7 @@ static void plan_tail(csv_plan* p) {
     // 4.53 ms against 4.73 for the two kernels back to back); with little decode work beside long chunks (configs[4]: 0.16)
     // giving SMs to the decode role for the whole launch costs more than it hides (8-layer step 46.1 against 44.4 ms), and
     // csv_tail_step keeps the two kernels.
-    const char* force = getenv("CSV_TAIL_DECODE_CTAS");   // tuning override: the decode-role CTAs of the one launch
+    const int32_t force = csv_tuning().v[CSV_TUNE_TAIL_DECODE_CTAS];   // tuning override: the decode-role CTAs of the one launch
     if (td < 0.25 * (td + ta) && !force) return;
     // A decode side that is too small costs more than one that is too large (SMs that finish their decode share take chunk
     // items, while a chunk-role SM can only take over a whole share), so the split leans 8 % towards decode.
@@ -177,7 +194,7 @@ static void plan_tail(csv_plan* p) {
     k = std::max(1, std::min(k, std::min(p->num_sms - 1, (p->num_sms * 3) / 4)));
     const int64_t want = (units + 8 * 4 - 1) / (8 * 4);
     k = (int)std::min<int64_t>(k, std::max<int64_t>(1, want));
-    if (force) k = std::max(1, std::min(p->num_sms - 1, atoi(force)));
+    if (force) k = std::max(1, std::min(p->num_sms - 1, force));
     p->tail_n_dec = k;
     // shares per decode-role SM (measured on configs[2] / [4]: 1 share 4.64 / 5.07 ms, 4 shares 4.98 / 5.26 ms: every share
     // ends with a CTA-wide barrier and restarts the rings)
@@ -290,7 +307,7 @@ static void plan_layout(csv_plan* p) {
     L.tail_items = take(p->tail_items.size() * sizeof(DecodeItem));
     L.tail_worker_begin = take(p->tail_worker_begin.size() * sizeof(int32_t));
     L.tail_groups = take(p->tail_groups.size() * sizeof(MergeGroup));
-    L.append_sched = take(128);   // zero in the uploaded image; the kernel's last CTA zeroes it again
+    L.append_sched = take(128);   // zero in the uploaded image; every launcher zeroes it again (cudaMemsetAsync) before its kernel
     std::vector<int32_t> meta;
     meta.insert(meta.end(), p->q_start.begin(), p->q_start.end());
     meta.insert(meta.end(), p->kv_lens.begin(), p->kv_lens.end());
@@ -350,6 +367,7 @@ csv_plan* csv_plan_build_host(const csv_attn_shape* shape, const int32_t* h_q_le
     for (int b = 0; b < batch; ++b) p->q_start[(size_t)b + 1] = p->q_start[(size_t)b] + h_q_lens[b];
     p->total_q = (int32_t)total_q;
     p->d_ws = nullptr;
+    p->tail_two_kernels = csv_tuning().v[CSV_TUNE_TAIL_TWO_KERNELS] != 0;
     // d = 128: 7 warp-workers x 2 ring stages per SM (112 KB in flight).  Measured against 8 x 3 (192 KB): configs[1] 184.8
     // against 201.2 us, configs[2] 2.02 against 2.12 ms, configs[4] 1.25 against 1.31 ms per layer (6 x 2: 184.8 us / 2.02 /
     // 1.23 ms): more bytes in flight than the latency needs only queue up in the memory system.
@@ -373,6 +391,16 @@ size_t csv_plan_workspace_bytes(const csv_attn_shape* shape, const int32_t* h_q_
     const size_t n = p->lay.total;
     delete p;
     return n;
+}
+
+int csv_tuning_set(int32_t knob, int32_t value) {
+    if (knob < 0 || knob > CSV_TUNE_TAIL_TWO_KERNELS || value < 0 || value > (1 << 20)) return CSV_E_INVAL;
+    csv_tuning().v[knob] = value;
+    return CSV_OK;
+}
+
+int32_t csv_tuning_get(int32_t knob) {
+    return (knob < 0 || knob > CSV_TUNE_TAIL_TWO_KERNELS) ? -1 : csv_tuning().v[knob];
 }
 
 int csv_plan_destroy(csv_plan_t* plan) {

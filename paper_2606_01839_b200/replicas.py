@@ -117,7 +117,18 @@ class PeerPools:
                 self._pools[key] = (local_pool, None)
             else:
                 ptr = B.csv_ipc_open(ticket["handle"], ticket["offset"])
-                self._pools[key] = (B.KvPool(desc, ptr, B.kv_pool_bytes(desc)), ptr)
+                # shape and offset arrived with the handle: the pool they describe must lie inside what was really mapped,
+                # else a "valid" block id of an oversized descriptor is a store outside the decoder's allocation
+                need = B.kv_pool_bytes(desc)
+                try:
+                    have = B.csv_ipc_mapped_bytes(ptr)
+                    if need == 0 or need > have:
+                        raise ValueError("ticket: a pool of shape %r needs %d bytes, the mapped allocation has %d after the "
+                                         "offset" % ((NL, nb, Hkv, d), need, have))
+                except Exception:
+                    B.csv_ipc_close(ptr)
+                    raise
+                self._pools[key] = (B.KvPool(desc, ptr, need), ptr)
         return self._pools[key][0]
 
     def push(self, ticket, d_k, d_v, d_ids=None, stream=None, local_pool=None):

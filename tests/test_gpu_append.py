@@ -231,6 +231,46 @@ def test_tail_step_mixed_batch_one_call(oracle):
         B.csv_tail_step(plan, sc.pool, layer, u16_dev(q), None, u16_dev(v_new), sc.d_tables, sc.max_blocks, d_out, d_lse)
 
 
+def test_tail_step_both_routes_in_one_process_against_the_oracle(oracle):
+    """csv_tail_step has two routes for a mixed step at d = 128: ONE persistent launch (tail_fused.cu) or the decode and
+    append kernels back to back.  The planner picks by the decode share of the work; CSV_TUNE_TAIL_TWO_KERNELS /
+    CSV_TUNE_TAIL_DECODE_CTAS override it per plan.  Both routes, plus the forced one-launch route on a batch where the
+    planner declines it, run here in one process on the same cache and are each compared with the oracle."""
+    rng = np.random.default_rng(97)
+    Hq, Hkv, d = 32, 8, 128
+    convs = [(3000, 1), (6000, 1), (500, 96), (4100, 1), (2500, 1), (1200, 300), (5000, 1), (15, 1)]
+    q_lens, kv_lens = [m for _, m in convs], [P + m for P, m in convs]
+    sc = Scenario(oracle, rng, Hq, Hkv, d, kv_lens).commit().upload()
+    q = synth.normal_bf16(rng, (sum(q_lens), Hq, d))
+    O_ref, LSE_ref = oracle_attention(sc, q_lens, q)
+    try:
+        O1, L1, info1 = run_attention(sc, q_lens, q, which="tail")
+        assert info1["tail_n_dec"] > 0                                   # decode-heavy batch: the planner fuses
+        assert_close(O1, L1, O_ref, LSE_ref, "one launch")
+        B.csv_tuning_set(B.TUNE_TAIL_TWO_KERNELS, 1)
+        O2, L2, info2 = run_attention(sc, q_lens, q, which="tail")
+        assert_close(O2, L2, O_ref, LSE_ref, "two kernels")
+        Ob, Lb, _ = run_attention(sc, q_lens, q, which="both")           # the two public calls: the very same kernels
+        assert np.array_equal(O2, Ob) and np.array_equal(L2, Lb)
+        B.csv_tuning_set(B.TUNE_TAIL_TWO_KERNELS, 0)
+        # a chunk-heavy batch: the planner keeps the two kernels; forcing 20 decode-role CTAs gives the one launch
+        convs = [(2000, 1), (9000, 700), (64, 1)]
+        q_lens, kv_lens = [m for _, m in convs], [P + m for P, m in convs]
+        sc = Scenario(oracle, rng, Hq, Hkv, d, kv_lens).commit().upload()
+        q = synth.normal_bf16(rng, (sum(q_lens), Hq, d))
+        O_ref, LSE_ref = oracle_attention(sc, q_lens, q)
+        O3, L3, info3 = run_attention(sc, q_lens, q, which="tail")
+        assert info3["tail_n_dec"] == 0
+        assert_close(O3, L3, O_ref, LSE_ref, "planner's choice: two kernels")
+        B.csv_tuning_set(B.TUNE_TAIL_DECODE_CTAS, 20)
+        O4, L4, info4 = run_attention(sc, q_lens, q, which="tail")
+        assert info4["tail_n_dec"] >= 1
+        assert_close(O4, L4, O_ref, LSE_ref, "one launch, forced")
+    finally:
+        for k in (B.TUNE_TAIL_TWO_KERNELS, B.TUNE_TAIL_DECODE_CTAS):
+            B.csv_tuning_set(k, 0)
+
+
 def test_tail_step_host_mixed_batch_two_layers(oracle):
     """csv_tail_step_host with q_lens and n_layers = 2: one plan, one table upload, both layers' new rows written, decode
     rows and appended chunks attended on each layer; host results against the oracle, whole pool against its scatter."""

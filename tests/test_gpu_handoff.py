@@ -202,6 +202,15 @@ def _prefiller_process(ticket, seed, q):
         keep = peers.push(ticket, u16_dev(K), u16_dev(V))
         torch.cuda.synchronize()
         ptr = peers._pools[next(iter(peers._pools))][1]
+        assert B.csv_ipc_mapped_bytes(ptr) >= B.kv_pool_bytes(B.pool_desc(NL, nb, Hkv, d))
+        # a ticket whose shape claims more memory than the decoder really shared is refused before any pool exists
+        # (shape and offset arrive in the same message as the handle), and its mapping reference is given back
+        big = dict(ticket, decoder=7, shape=(NL, nb * 4096, Hkv, d))
+        with pytest.raises(ValueError, match="mapped allocation"):
+            peers.get(big)
+        assert len(peers._pools) == 1
+        with pytest.raises(B.CsvError):
+            B.csv_ipc_mapped_bytes(ptr + 128)                      # not a pointer csv_ipc_open handed out
         peers.close()
         with pytest.raises(B.CsvError):
             B.csv_ipc_close(ptr)                                   # unknown pointer now

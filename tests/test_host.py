@@ -300,6 +300,37 @@ def test_mixed_step_split_follows_the_work():
     assert split([1] * 200 + [2], [60000] * 200 + [64])[0] <= 111        # never more than 3/4 of the SMs on decode
 
 
+def test_tuning_knobs_are_read_at_plan_build_and_recorded_in_the_plan():
+    # the overrides were getenv calls inside the planner (every build) and a cached static in csv_tail_step.  They
+    # are now one process-wide table that a test can flip; a plan keeps what it was built with.
+    sh = B.attn_shape(64, 8, 128)
+    c5q, c5kv = [1] * 16 + [256] * 4, [131072] * 20
+    try:
+        assert [B.csv_tuning_get(k) for k in (0, 1, 2)] == [0, 0, 0] and B.csv_tuning_get(3) == -1
+        base = B.Plan(sh, c5q, c5kv)
+        assert base.info()["tail_n_dec"] == 0 and base.info()["decode_grid"] == 148
+        ws_default = B.csv_plan_workspace_bytes(sh, c5q, c5kv)
+        B.csv_tuning_set(B.TUNE_TAIL_DECODE_CTAS, 26)                   # force the one-launch route where the planner declines it
+        forced = B.Plan(sh, c5q, c5kv)
+        assert forced.info()["tail_n_dec"] == 26 and forced.info()["tail_n_shares"] == 26
+        assert B.csv_plan_workspace_bytes(sh, c5q, c5kv) >= ws_default  # the size query sees the same table as the build
+        assert base.info()["tail_n_dec"] == 0                           # existing plans keep what they were built with
+        B.csv_tuning_set(B.TUNE_TAIL_DECODE_CTAS, 10 ** 5)
+        assert B.Plan(sh, c5q, c5kv).info()["tail_n_dec"] == 147        # always one CTA left for the other role
+        B.csv_tuning_set(B.TUNE_TAIL_DECODE_CTAS, 0)
+        assert B.Plan(sh, c5q, c5kv).info()["tail_n_dec"] == 0
+        B.csv_tuning_set(B.TUNE_DECODE_GRID, 37)
+        assert B.Plan(sh, c5q, c5kv).info()["decode_grid"] == 37
+        assert B.Plan(sh, [1], [16]).info()["decode_grid"] == 1         # a cap, not a floor
+        for bad in ((-1, 1), (3, 1), (0, -5), (1, (1 << 20) + 1)):
+            with pytest.raises(B.CsvError):
+                B.csv_tuning_set(*bad)
+    finally:
+        for k in (0, 1, 2):
+            B.csv_tuning_set(k, 0)
+    assert B.Plan(sh, c5q, c5kv).info()["decode_grid"] == 148
+
+
 def test_handoff_direct_and_ipc_reject_bad_arguments_before_touching_cuda():
     pool = mkpool(8, NL=1, Hkv=1, d=64)
     k = FAKE + (1 << 20)
@@ -324,7 +355,44 @@ def test_handoff_direct_and_ipc_reject_bad_arguments_before_touching_cuda():
     assert L.csv_ipc_open(None, 0, ctypes.byref(out)) == B.CSV_E_INVAL
     assert L.csv_ipc_open(buf, 0, None) == B.CSV_E_INVAL
     assert L.csv_ipc_close(ctypes.c_void_p(k)) == B.CSV_E_INVAL                   # never opened
+    nbytes = ctypes.c_size_t(77)
+    assert L.csv_ipc_mapped_bytes(ctypes.c_void_p(k), ctypes.byref(nbytes)) == B.CSV_E_INVAL   # not a csv_ipc_open pointer
+    assert L.csv_ipc_mapped_bytes(None, ctypes.byref(nbytes)) == B.CSV_E_INVAL
+    assert L.csv_ipc_mapped_bytes(ctypes.c_void_p(k), None) == B.CSV_E_INVAL and nbytes.value == 77
     assert pool.used_blocks == 0
+
+
+def test_tail_step_host_refuses_bad_lengths_before_any_copy_is_enqueued():
+    # q_len > kv_len used to be found by the planner AFTER the four host->device copies were enqueued.  On this
+    # box there is no GPU, so a call that reached cudaMemcpyAsync would come back CSV_E_CUDA: CSV_E_INVAL proves the order.
+    pool = mkpool(64, NL=2)
+    sh = B.attn_shape(32, 8, 128)
+
+    class FakeBuf:   # what binding._ptr / workspace sizing need from a tensor
+        def __init__(self, ptr, n):
+            self.ptr, self.n = ptr, n
+
+        def data_ptr(self):
+            return self.ptr
+
+        def numel(self):
+            return self.n
+
+        def element_size(self):
+            return 1
+
+    ws = FakeBuf(FAKE, 1 << 30)
+    h = FakeBuf(FAKE + (1 << 31), 1 << 20)
+    call = lambda kv, q=None, mpt=0, shape=sh: B.csv_tail_step_host(pool, 0, shape, kv, h, h, h, h, 8, ws, h, h, mpt, stream=0,
+                                                                     q_lens=q, n_layers=2)
+    for bad in (lambda: call([100, 50], [1, 51]),            # q_len > kv_len
+                lambda: call([100, -1]),                      # negative length
+                lambda: call([100, 0], [1, 2]),               # only a DECODE row may sit on an empty cache
+                lambda: call([100, 50], mpt=24),              # partition size not a multiple of 16
+                lambda: call([100, 50], shape=B.attn_shape(24, 8, 128))):   # G = 3
+        with pytest.raises(B.CsvError) as e:
+            bad()
+        assert e.value.code == B.CSV_E_INVAL
 
 
 def test_committed_ncu_traffic_rows_belong_to_the_current_kernel_sources():
