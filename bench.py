@@ -248,17 +248,23 @@ def oracle_eval(item, wl):
     return res
 
 
-def parity_of(wl, results):
-    """max |O err| and |LSE err| of the device outputs (wl.d_out / wl.d_lse as they stand) on the oracle's rows."""
+def parity_of(wl, results, out=None, lse=None):
+    """max |O err| and |LSE err| on the oracle's rows of the device outputs (wl.d_out / wl.d_lse as they stand), or of the
+    given tensors (e.g. the host buffers a csv_tail_step_host loop filled: same [total_q] row order)."""
     from paper_2606_01839_b200 import synth
 
-    O = wl.d_out.cpu().numpy().view(np.uint16)
-    LSE = wl.d_lse.cpu().numpy().astype(np.float64)
+    O = (wl.d_out if out is None else out).cpu().reshape(-1, wl.Hq, wl.d).numpy().view(np.uint16)
+    LSE = (wl.d_lse if lse is None else lse).cpu().reshape(-1, wl.Hq).numpy().astype(np.float64)
     eo = el = 0.0
     for r, n, o, l in results:
         eo = max(eo, float(np.abs(synth.bf16_bits_to_f32(O[r]).astype(np.float64) - o).max()))
         el = max(el, float(np.abs(LSE[r] - l).max()))
     return eo, el
+
+
+def route_record(route, eo, el):
+    """One entry of parity.routes: the route that was TIMED, checked on its own output."""
+    return {"route": route, "max_abs_err_O": eo, "max_abs_err_LSE": el, "ok": bool(eo <= O_TOL and el <= LSE_TOL)}
 
 
 def oracle_timed(wl, picks, threads, layer=0):
@@ -360,6 +366,7 @@ def leg_long_context(args, rank, world, ranks_on_dev, dist, agg_dev, pk, sampler
     e2e_ms, _ = replicas.aggregate(dist, e2e_ms, 0, device=agg_dev)
     h2d = (h_q.numel() + h_k.numel() + h_v.numel()) * 2 + h_t.numel() * 4
     d2h = h_out.numel() * 2 + h_lse.numel() * 4
+    wl.e2e_layer0 = (h_out[0].clone(), h_lse[0].clone())   # the last host-buffer step's result (layer 0): checked by run_ours
     del ws, h_q, h_k, h_v, h_out, h_lse
 
     value = total_bytes / ms_step / 1e6
@@ -381,7 +388,7 @@ def leg_long_context(args, rank, world, ranks_on_dev, dist, agg_dev, pk, sampler
         "gpu_launches": 2 * L * K, "clocks": clocks,
     }
     head = roofline_block("decode_kernel", "configs[4]", "hbm", kv_layer, dec, pk,
-                          note="per paged_decode_attn call (decode_kernel<128,3,8> + decode_merge_kernel), one layer = 8.59 GB; "
+                          note="per paged_decode_attn call (decode_kernel<128,2,7> + decode_merge_kernel), one layer = 8.59 GB; "
                                "calls cycle over the %d resident layers" % L)
     return fields, head, wl, L
 
@@ -430,8 +437,21 @@ def leg_long_context_extras(wl, L, pk, iters=6):
                     "1000 W cap (sw_power_cap), where the same calls are 10-13 %% slower whichever way they are launched "
                     "(separate_calls_ms is the like-for-like figure); decode_role_ctas 0 = the plan kept the two-kernel route "
                     "(decode is under a quarter of this step)" % L}
-    del mixed
-    return blocks, [step], app
+    # for the live parity of the timed route: layer 0 through the plan's own route, and the same batch and queries through
+    # the ONE-launch route forced by the tuning knob (a twin plan over the same pool)
+    from paper_2606_01839_b200 import binding as B
+    mixed.d_out.fill_(0x7FC0)
+    mixed.tail_attn(layer=0)
+    try:
+        B.csv_tuning_set(B.TUNE_TAIL_DECODE_CTAS, 26)
+        forced = mixed.with_q_lens(mixed.q_lens)
+    finally:
+        B.csv_tuning_set(B.TUNE_TAIL_DECODE_CTAS, 0)
+    forced.d_q.copy_(mixed.d_q)
+    forced.d_out.fill_(0x7FC0)
+    forced.tail_attn(layer=0)
+    torch.cuda.synchronize()
+    return blocks, [step], app, mixed, forced
 
 
 def leg_c2(args, pk, dist, agg_dev):
@@ -487,9 +507,26 @@ def leg_c2(args, pk, dist, agg_dev):
             "decode_items": info["n_decode_items"]}
     block = roofline_block("decode_kernel", "configs[1]", "hbm", kv_bytes, dec, pk,
                            note="per paged_decode_attn call (decode_kernel + decode_merge_kernel)")
-    del wl, big
+    # The WHOLE config through the oracle on one core ("c1, c2: the whole config"), timed, and compared with the
+    # output of the route that was timed (paged_decode_step); then the host-buffer loop's last step (kv_len = base + 104,
+    # h_out / h_lse as the call left them) on 8 conversations.  The oracle reads the pool back as the steps left it.
+    wl.d_out.fill_(0x7FC0)
+    wl.decode_step()
+    torch.cuda.synchronize()
+    dt, th, res = oracle_timed(wl, [(b, [0]) for b in range(rows)], 1)
+    routes = [route_record("paged_decode_step, configs[1], whole config (64 conversations x 32 heads)", *parity_of(wl, res))]
+    last = big.with_q_lens([1] * rows, kv_lens=[t + 104 for t in base])
+    last.d_q.copy_(wl.d_q)
+    _, _, res_last = oracle_timed(last, [(b, [0]) for b in range(0, rows, 8)], 1)
+    routes.append(route_record("csv_tail_step_host, configs[1], step 105 of the host-buffer decode loop (h_out / h_lse)",
+                               *parity_of(last, res_last, h_out, h_lse)))
+    cpu = {"config": "configs[1]", "kind": "oracle", "cores": 1, "value": kv_bytes / dt / 1e9, "unit": UNIT, "seconds": dt,
+           "sample": "the whole config: 64 conversations, all 32 heads, once",
+           "parity_max_abs_err": max(r["max_abs_err_O"] for r in routes),
+           "parity_max_lse_err": max(r["max_abs_err_LSE"] for r in routes), "parity_routes": routes}
+    del wl, big, last
     torch.cuda.empty_cache()
-    return [block], [step]
+    return [block], [step], cpu
 
 
 def leg_c3(args, pk, with_oracle):
@@ -550,20 +587,31 @@ def leg_c3(args, pk, with_oracle):
     cpu = None
     if with_oracle:
         # sampled oracle, extrapolated by KV token-heads: 8 decode rows, 2 chunks x 4 rows
-        wl.decode()
-        wl.append()
+        # the timed route first: csv_tail_step (KV write + the one persistent launch), checked on its OWN output; then
+        # the host-buffer call's h_out / h_lse as the last timed iteration left them; then the two standalone calls
+        wl.d_out.fill_(0x7FC0)
+        wl.tail_step()
         torch.cuda.synchronize()
         dec_rows = [b for b, q in enumerate(wl.q_lens) if q == 1][:8]
         chunks = [b for b, q in enumerate(wl.q_lens) if q > 1][:2]
         picks = [(b, [0]) for b in dec_rows] + [(b, [0, wl.q_lens[b] // 3, (2 * wl.q_lens[b]) // 3, wl.q_lens[b] - 1]) for b in chunks]
         dt, th, res = oracle_timed(wl, picks, 1)
-        eo, el = parity_of(wl, res)
+        routes = [route_record("csv_tail_step, configs[2] (one launch, decode_role_ctas %d)" % wl.plan.info()["tail_n_dec"],
+                               *parity_of(wl, res)),
+                  route_record("csv_tail_step_host, configs[2], last timed host-buffer step (h_out / h_lse)",
+                               *parity_of(wl, res, h_out, h_lse))]
+        wl.d_out.fill_(0x7FC0)
+        wl.decode()
+        wl.append()
+        torch.cuda.synchronize()
+        routes.append(route_record("paged_decode_attn + append_prefill_attn, configs[2] (the roofline blocks' calls)", *parity_of(wl, res)))
+        eo, el = max(r["max_abs_err_O"] for r in routes), max(r["max_abs_err_LSE"] for r in routes)
         all_th = sum(kv for q, kv in zip(wl.q_lens, wl.kv_lens) if q == 1) * wl.Hq
         all_th += sum(q * (kv - q) + q * (q + 1) // 2 for q, kv in zip(wl.q_lens, wl.kv_lens) if q > 1) * wl.Hq
         cpu = {"config": "configs[2]", "kind": "oracle", "cores": 1, "sample": "8 decode rows + 2 chunks x 4 rows, all 32 heads",
                "sample_seconds": dt, "sample_token_heads": th, "extrapolated_step_seconds": dt * all_th / th,
                "extrapolated": True, "basis": "KV token-heads scanned (%.3g in the step)" % all_th,
-               "parity_max_abs_err": eo, "parity_max_lse_err": el}
+               "parity_max_abs_err": eo, "parity_max_lse_err": el, "parity_routes": routes}
     del wl
     torch.cuda.empty_cache()
     return blocks, [step], cpu
@@ -811,7 +859,10 @@ def run_ours(args):
     rooflines, steps, cpus = [head], [], []
     if world == 1:
         # ---- CPU baseline: the oracle as it stands on a bounded sample of the headline workload (layer 0) -------------
-        wl.decode(layer=0)
+        # the route that was timed: paged_decode_step (the new token's KV write inside the decode launch).  It leaves the
+        # token in the pool, and the oracle reads the pool back afterwards, so the write is part of what is checked.
+        wl.d_out.fill_(0x7FC0)
+        wl.decode_step(layer=0)
         torch.cuda.synchronize()
         cores = len(os.sched_getaffinity(0))
         dt1, th1, res1 = oracle_timed(wl, [(b, [0]) for b in range(4)], 1)
@@ -821,6 +872,14 @@ def run_ours(args):
         dtn, thn, resn = oracle_timed(wl, [(b, [0]) for b in range(nall)], cores)
         eo2, el2 = parity_of(wl, resn)
         eo, el = max(eo, eo2), max(el, el2)
+        routes = [route_record("paged_decode_step, configs[4] layer 0 (the headline step's call), %d conversations" % nall, eo, el)]
+        routes.append(route_record("csv_tail_step_host, configs[4] layer 0 of the last timed host-buffer step (h_out / h_lse)",
+                                   *parity_of(wl, resn, *wl.e2e_layer0)))
+        wl.d_out.fill_(0x7FC0)
+        wl.decode(layer=0)
+        torch.cuda.synchronize()
+        routes.append(route_record("paged_decode_attn, configs[4] layer 0 (the roofline block's call)", *parity_of(wl, resn)))
+        eo, el = max(r["max_abs_err_O"] for r in routes), max(r["max_abs_err_LSE"] for r in routes)
         nbn = nall * wl.kv_lens[0] * wl.Hkv * wl.d * 4
         line["cpu_baseline"] = {"value": nb1 / dt1 / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": dt1,
                                 "sample": "4 of the 16 conversations of configs[4], layer 0 (%.1f GB of KV), all 64 heads, once" % (nb1 / 1e9),
@@ -833,7 +892,7 @@ def run_ours(args):
                      "sample_seconds": dt1})
         line["parity"] = {"config": "configs[4] layer 0, %d conversations x 64 heads against the oracle" % nall,
                           "max_abs_err_O": eo, "max_abs_err_LSE": el, "gate_O": O_TOL, "gate_LSE": LSE_TOL,
-                          "ok": bool(eo <= O_TOL and el <= LSE_TOL)}
+                          "ok": bool(eo <= O_TOL and el <= LSE_TOL), "routes": routes}
         if not args.no_extras:
             def guarded(name, fn):
                 try:
@@ -846,7 +905,7 @@ def run_ours(args):
             if r:
                 rooflines += r[0]
                 steps += r[1]
-                app = r[2]
+                app, mixed, forced = r[2], r[3], r[4]
                 # two sampled rows of one appended chunk through the oracle, extrapolated to the step
                 try:
                     app.append(layer=0)
@@ -860,9 +919,21 @@ def run_ours(args):
                     line["parity"]["append_sample_max_abs_err_O"] = ea
                     line["parity"]["append_sample_max_abs_err_LSE"] = ela
                     line["parity"]["ok"] = bool(line["parity"]["ok"] and ea <= O_TOL and ela <= LSE_TOL)
-                except Exception as e:
+                    # the mixed step as timed (csv_tail_step per layer): one decode row + rows 0 and 255 of chunk entry 16
+                    # (an alias of conversation 0), on the plan's route and on the forced one-launch route
+                    _, _, resm = oracle_timed(mixed, [(5, [0]), (16, [0, 255])], 1)
+                    for w, name in ((mixed, "csv_tail_step, configs[4] mixed step layer 0, the plan's route (decode_role_ctas %d)"
+                                     % mixed.plan.info()["tail_n_dec"]),
+                                    (forced, "csv_tail_step, configs[4] mixed step layer 0, one launch forced (decode_role_ctas %d)"
+                                     % forced.plan.info()["tail_n_dec"])):
+                        line["parity"]["routes"].append(route_record(name, *parity_of(w, resm)))
+                    line["parity"]["routes"].append(route_record("append_prefill_attn, configs[4] layer 0 (the roofline block's call)", ea, ela))
+                    line["parity"]["ok"] = bool(line["parity"]["ok"] and all(r["ok"] for r in line["parity"]["routes"]))
+                except Exception as e:   # an extra must never cost the headline line: the route is listed as unchecked
                     sys.stderr.write("append oracle sample failed: %r\n" % (e,))
-                del app
+                    line["parity"]["routes"].append({"route": "configs[4] appended chunks / mixed step", "ok": None,
+                                                     "unchecked": repr(e)[:200]})
+                del app, mixed, forced
         del wl
         torch.cuda.empty_cache()
         if not args.no_extras:
@@ -873,6 +944,7 @@ def run_ours(args):
                     rooflines += r[0]
                     steps += r[1]
                     if len(r) > 2 and r[2]:
+                        line["parity"]["routes"] += r[2].pop("parity_routes", [])
                         cpus.append(r[2])
                         line["parity"]["ok"] = bool(line["parity"]["ok"] and r[2].get("parity_max_abs_err", 0) <= O_TOL and
                                                     r[2].get("parity_max_lse_err", 0) <= LSE_TOL)

@@ -18,20 +18,54 @@ def free_gb():
     return torch.cuda.mem_get_info()[0] / 1e9
 
 
-def check_rows(oracle, wl, layer, samples, O, LSE, what):
-    """samples: list of (conversation b, row index i inside its q rows).  Oracle on the truncated cache."""
+def check_rows(oracle, wl, layer, samples, O, LSE, what, written=False):
+    """samples: list of (conversation b, row index i inside its q rows).  Oracle on the truncated cache.
+    written: the step under test also WROTE the new rows' K/V (csv_tail_step / paged_decode_step): the rows the oracle
+    gathers back from the pool at positions [kv_len - m, kv_len) must then be the step's k_new / v_new, bit for bit."""
     starts = np.concatenate([[0], np.cumsum(wl.q_lens)])
     q_all = dev_to_u16(wl.d_q).reshape(-1, wl.Hq, wl.d)
     cache = {}
     for b, i in samples:
         if b not in cache:
             cache = {b: logical_kv(oracle, wl, b, layer)}     # keep one conversation at a time (131k tokens = 512 MiB)
+            if written:
+                m, t = wl.q_lens[b], wl.kv_lens[b]
+                per_layer = wl.total_q * wl.Hkv * wl.d
+                lo, hi = layer * per_layer + starts[b] * wl.Hkv * wl.d, layer * per_layer + (starts[b] + m) * wl.Hkv * wl.d
+                for name, new, got in (("K", wl.d_k_new, cache[b][0]), ("V", wl.d_v_new, cache[b][1])):
+                    want = dev_to_u16(new[lo:hi]).reshape(m, wl.Hkv, wl.d)
+                    assert np.array_equal(got[t - m:t], want), "%s conv %d: new %s rows are not in the pool" % (what, b, name)
         K, V = cache[b]
         m = wl.q_lens[b]
         n = wl.kv_lens[b] - m + i + 1                        # keys visible to row i (decode: m = 1, i = 0, n = kv_len)
         r = starts[b] + i
         o_ref, l_ref = oracle.attention(q_all[r:r + 1], K[:n], V[:n])
         assert_close(O[r:r + 1], LSE[r:r + 1], o_ref, l_ref, what="%s conv %d row %d (n=%d)" % (what, b, i, n))
+
+
+def seeded_samples(wl, rng, n_decode, n_append_convs, rows_per_chunk):
+    """(b, i) samples chosen by a seeded RNG: n_decode decode rows; rows_per_chunk rows (first, last, random) of each of
+    n_append_convs chunks.  Grouped by conversation so that check_rows loads each cache once."""
+    dec = [b for b, m in enumerate(wl.q_lens) if m == 1]
+    app = [b for b, m in enumerate(wl.q_lens) if m > 1]
+    out = [(int(b), 0) for b in rng.choice(dec, size=min(n_decode, len(dec)), replace=False)]
+    for b in rng.choice(app, size=min(n_append_convs, len(app)), replace=False) if app else []:
+        m = wl.q_lens[b]
+        rows = {0, m - 1} | {int(x) for x in rng.integers(0, m, size=max(0, rows_per_chunk - 2))}
+        out += [(int(b), i) for i in sorted(rows)]
+    return out
+
+
+def outputs(wl):
+    torch.cuda.synchronize()
+    O, LSE = bf16_dev_to_f64(wl.d_out), wl.d_lse.cpu().numpy().astype(np.float64)
+    assert np.all(np.isfinite(O)) and np.all(np.isfinite(LSE)), "a row was left unwritten"
+    return O, LSE
+
+
+def poison_outputs(wl):
+    wl.d_out.fill_(0x7FC0)
+    wl.d_lse.fill_(float("nan"))
 
 
 def test_config3_agentic_tail_mix_full_size(oracle):
@@ -57,6 +91,37 @@ def test_config3_agentic_tail_mix_full_size(oracle):
     check_rows(oracle, wl, 0, samples, O, LSE, "config 3")
 
 
+def test_config3_timed_route_one_launch_tail_step_full_size(oracle):
+    """What bench.py times on configs[2] is csv_tail_step: the KV write of all 9k new rows, then ONE persistent launch
+    whose work items are the 224 decode rows' shares and the 32 chunks' tiles (the timed path must be the
+    checked path).  Seeded sample of 16 decode rows and 8 chunks x 4 rows against the oracle, the written rows bit for bit,
+    and a second run bit-identical to the first."""
+    wl = workloads.config_tail_workload(3)
+    assert wl.plan.info()["tail_n_dec"] > 0                              # the plan takes the one-launch route here
+    poison_outputs(wl)
+    wl.tail_step()
+    O, LSE = outputs(wl)
+    samples = seeded_samples(wl, np.random.default_rng(303), 16, 8, 4)
+    assert sum(1 for b, _ in samples if wl.q_lens[b] == 1) >= 16 and sum(1 for b, _ in samples if wl.q_lens[b] > 1) >= 24
+    check_rows(oracle, wl, 0, samples, O, LSE, "config 3 csv_tail_step", written=True)
+    first = (wl.d_out.clone(), wl.d_lse.clone())
+    poison_outputs(wl)
+    wl.tail_step()
+    torch.cuda.synchronize()
+    assert torch.equal(first[0], wl.d_out) and torch.equal(first[1], wl.d_lse), "csv_tail_step differs from run to run"
+    # the two-kernel route on the same plan inputs (a plan built with the override): within tolerance of the same oracle rows
+    try:
+        B.csv_tuning_set(B.TUNE_TAIL_TWO_KERNELS, 1)
+        two = wl.with_q_lens(wl.q_lens)
+    finally:
+        B.csv_tuning_set(B.TUNE_TAIL_TWO_KERNELS, 0)
+    two.d_q.copy_(wl.d_q)
+    poison_outputs(two)
+    two.tail_attn()
+    O2, LSE2 = outputs(two)
+    check_rows(oracle, two, 0, samples[:6] + samples[-6:], O2, LSE2, "config 3 two-kernel route")
+
+
 def test_config5_long_context_full_size_eight_layers(oracle):
     # BASELINE.json config 5: Hq=64, Hkv=8, d=128, 8 layers, 16 x 131072 tokens (~69 GB of KV), >= 64 partitions per sequence
     if free_gb() < 90:
@@ -66,19 +131,43 @@ def test_config5_long_context_full_size_eight_layers(oracle):
     items, _ = wl.plan.decode_items()
     assert np.bincount(items[:, 0], minlength=16).min() >= 64
     app = wl.with_q_lens(workloads.config5_append_q_lens())
-    for layer in (0, 7):                                     # layer 7 starts 56 GiB into the pool: 64-bit addressing
-        wl.d_out.fill_(0x7FC0)
-        wl.decode(layer=layer)
-        torch.cuda.synchronize()
-        O, LSE = bf16_dev_to_f64(wl.d_out), wl.d_lse.cpu().numpy().astype(np.float64)
-        assert np.all(np.isfinite(O))
-        check_rows(oracle, wl, layer, [(3 if layer == 0 else 15, 0)], O, LSE, "config 5 decode layer %d" % layer)
-    app.d_out.fill_(0x7FC0)
+    rng = np.random.default_rng(505)
+    # the headline route: paged_decode_step (KV write of the new token inside the decode launch) on three layers; layer 7
+    # starts 56 GiB into the pool (64-bit addressing).  9 seeded rows in all, the written token checked bit for bit.
+    for layer, n_rows in ((0, 3), (3, 3), (7, 3)):
+        poison_outputs(wl)
+        wl.decode_step(layer=layer)
+        O, LSE = outputs(wl)
+        rows = [(int(b), 0) for b in rng.choice(16, size=n_rows, replace=False)]
+        check_rows(oracle, wl, layer, rows, O, LSE, "config 5 paged_decode_step layer %d" % layer, written=True)
+    poison_outputs(wl)
+    wl.decode(layer=7)                                      # the plain call on the same cache: same kernel without the write
+    O, LSE = outputs(wl)
+    check_rows(oracle, wl, 7, [(15, 0)], O, LSE, "config 5 decode layer 7")
+    poison_outputs(app)
     app.append(layer=7)
     torch.cuda.synchronize()
     O, LSE = bf16_dev_to_f64(app.d_out), app.d_lse.cpu().numpy().astype(np.float64)
     assert np.all(np.isfinite(O))
     check_rows(oracle, app, 7, [(2, 0), (2, 255)], O, LSE, "config 5 append layer 7")
+    del app
+    # the mixed step bench.py times on configs[4] (16 decode rows + 4 chunks of 256 as ONE csv_tail_step): the route the
+    # plan picks (two kernels: the decode share is under a quarter), then the one-launch route forced on the same batch
+    mixed = wl.with_extra_chunks(synth.config_lengths(5)["append_convs"], synth.config_lengths(5)["m"])
+    assert mixed.plan.info()["tail_n_dec"] == 0
+    try:
+        B.csv_tuning_set(B.TUNE_TAIL_DECODE_CTAS, 26)
+        forced = mixed.with_q_lens(mixed.q_lens)
+    finally:
+        B.csv_tuning_set(B.TUNE_TAIL_DECODE_CTAS, 0)
+    assert forced.plan.info()["tail_n_dec"] == 26
+    for w, layer, chunk, what in ((mixed, 7, 16, "plan's route"), (forced, 0, 18, "one launch forced")):
+        poison_outputs(w)
+        w.tail_attn(layer=layer)
+        O, LSE = outputs(w)
+        m = w.q_lens[chunk]
+        rows = [(int(rng.integers(0, 16)), 0)] + [(chunk, i) for i in sorted({0, m - 1, int(rng.integers(1, m - 1)), int(rng.integers(1, m - 1))})]
+        check_rows(oracle, w, layer, rows, O, LSE, "config 5 csv_tail_step (%s) layer %d" % (what, layer))
 
 
 def test_config4_handoff_full_size(oracle):
