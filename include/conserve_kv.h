@@ -297,12 +297,18 @@ int kv_append_tokens(kv_pool_t* dst, const csv_plan_t* plan, const void* d_k_new
  *   CSV_TUNE_TAIL_DECODE_CTAS   decode-role CTAs of a mixed step's one launch, also where the planner would have kept
  *                               the two kernels (default: chosen from the two roles' work, conserve_kv.h csv_tail_step)
  *   CSV_TUNE_TAIL_TWO_KERNELS   non-zero: csv_tail_step never uses the one-launch route for plans built from now on
+ *   CSV_TUNE_SM_DECODE_GBS      GB/s ONE SM pulls in the decode role (default 75) and
+ *   CSV_TUNE_SM_APPEND_GFLOPS   GFLOP/s one SM sustains in the append role (default 7400): the two rates from which a
+ *                               mixed step's split is computed; a caller that calibrated its own device sets both
  * At first use each knob is initialised from the environment variable of the same name without "TUNE_"
- * (CSV_DECODE_GRID, CSV_TAIL_DECODE_CTAS: a positive decimal integer, anything else is ignored; CSV_TAIL_TWO_KERNELS:
- * any value other than 0).  Not thread-safe against concurrent plan builds.  csv_tuning_get returns -1 for a bad knob. */
+ * (CSV_DECODE_GRID, CSV_TAIL_DECODE_CTAS, CSV_SM_DECODE_GBS, CSV_SM_APPEND_GFLOPS: a positive decimal integer, anything
+ * else is ignored; CSV_TAIL_TWO_KERNELS: any value other than 0).  Not thread-safe against concurrent plan builds.  csv_tuning_get returns -1 for a bad knob. */
 #define CSV_TUNE_DECODE_GRID       0
 #define CSV_TUNE_TAIL_DECODE_CTAS  1
 #define CSV_TUNE_TAIL_TWO_KERNELS  2
+#define CSV_TUNE_SM_DECODE_GBS     3
+#define CSV_TUNE_SM_APPEND_GFLOPS  4
+#define CSV_TUNE_COUNT             5
 int csv_tuning_set(int32_t knob, int32_t value);
 int32_t csv_tuning_get(int32_t knob);
 

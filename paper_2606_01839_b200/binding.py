@@ -320,7 +320,7 @@ def csv_ipc_copy(dst, src, nbytes, stream=None):
     _check("csv_ipc_copy", lib().csv_ipc_copy(_ptr(dst), _ptr(src), int(nbytes), _stream(stream)))
 
 
-TUNE_DECODE_GRID, TUNE_TAIL_DECODE_CTAS, TUNE_TAIL_TWO_KERNELS = 0, 1, 2
+TUNE_DECODE_GRID, TUNE_TAIL_DECODE_CTAS, TUNE_TAIL_TWO_KERNELS, TUNE_SM_DECODE_GBS, TUNE_SM_APPEND_GFLOPS = 0, 1, 2, 3, 4
 
 
 def csv_tuning_set(knob, value):

@@ -146,7 +146,7 @@ int launch_append_attn_tc2(const csv_plan* plan, const kv_pool* pool, int layer,
 // Tuning knobs (conserve_kv.h csv_tuning_set): one process-wide table, initialised once from the environment; every plan
 // records what it was built with, so a plan and its workspace size cannot disagree unless the caller changes a knob between.
 struct CsvTuning {
-    int32_t v[3];   // indexed by CSV_TUNE_*; 0 = library default
+    int32_t v[CSV_TUNE_COUNT];   // indexed by CSV_TUNE_*; 0 = library default
 };
 CsvTuning& csv_tuning();
 int csv_query_num_sms();   // SM count of the current device, 148 if none is usable

@@ -35,7 +35,8 @@ static int32_t env_knob(const char* name, bool flag) {
 
 CsvTuning& csv_tuning() {
     static CsvTuning t = {{env_knob("CSV_DECODE_GRID", false), env_knob("CSV_TAIL_DECODE_CTAS", false),
-                           env_knob("CSV_TAIL_TWO_KERNELS", true)}};
+                           env_knob("CSV_TAIL_TWO_KERNELS", true), env_knob("CSV_SM_DECODE_GBS", false),
+                           env_knob("CSV_SM_APPEND_GFLOPS", false)}};
     return t;
 }
 
@@ -179,7 +180,12 @@ static void plan_tail(csv_plan* p) {
         if (m > 1) flops += 4.0 * d * Hq * m * ((double)(p->kv_lens[b] - m) + (m + 1) / 2.0);
     }
     const double bytes = (double)units * 2.0 * csv_tile_bytes(d);
-    const double sm_gbs = 75.0, sm_tflops = 7.4;   // one SM: decode role pulls ~75 GB/s, append role sustains 7.0-7.8 TFLOP/s
+    // one SM: the decode role pulls ~75 GB/s, the append role sustains 7.0-7.8 TFLOP/s (one B200 pool's numbers, DESIGN.md
+    // section 5: the best split moved between boxes).  A caller that has calibrated its own device passes its rates through
+    // csv_tuning_set; only their ratio matters here.
+    const CsvTuning& tune = csv_tuning();
+    const double sm_gbs = tune.v[CSV_TUNE_SM_DECODE_GBS] ? (double)tune.v[CSV_TUNE_SM_DECODE_GBS] : 75.0;
+    const double sm_tflops = tune.v[CSV_TUNE_SM_APPEND_GFLOPS] ? tune.v[CSV_TUNE_SM_APPEND_GFLOPS] / 1000.0 : 7.4;
     const double td = bytes / (sm_gbs * 1e9), ta = flops / (sm_tflops * 1e12);   // SM-seconds of each role
     // The one launch pays when the decode rows are a sizeable part of the step (configs[2]: td / (td + ta) = 0.34, one call
     // 4.53 ms against 4.73 for the two kernels back to back); with little decode work beside long chunks (configs[4]: 0.16)
@@ -394,13 +400,13 @@ size_t csv_plan_workspace_bytes(const csv_attn_shape* shape, const int32_t* h_q_
 }
 
 int csv_tuning_set(int32_t knob, int32_t value) {
-    if (knob < 0 || knob > CSV_TUNE_TAIL_TWO_KERNELS || value < 0 || value > (1 << 20)) return CSV_E_INVAL;
+    if (knob < 0 || knob >= CSV_TUNE_COUNT || value < 0 || value > (1 << 20)) return CSV_E_INVAL;
     csv_tuning().v[knob] = value;
     return CSV_OK;
 }
 
 int32_t csv_tuning_get(int32_t knob) {
-    return (knob < 0 || knob > CSV_TUNE_TAIL_TWO_KERNELS) ? -1 : csv_tuning().v[knob];
+    return (knob < 0 || knob >= CSV_TUNE_COUNT) ? -1 : csv_tuning().v[knob];
 }
 
 int csv_plan_destroy(csv_plan_t* plan) {

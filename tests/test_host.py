@@ -306,7 +306,7 @@ def test_tuning_knobs_are_read_at_plan_build_and_recorded_in_the_plan():
     sh = B.attn_shape(64, 8, 128)
     c5q, c5kv = [1] * 16 + [256] * 4, [131072] * 20
     try:
-        assert [B.csv_tuning_get(k) for k in (0, 1, 2)] == [0, 0, 0] and B.csv_tuning_get(3) == -1
+        assert [B.csv_tuning_get(k) for k in range(5)] == [0] * 5 and B.csv_tuning_get(5) == -1
         base = B.Plan(sh, c5q, c5kv)
         assert base.info()["tail_n_dec"] == 0 and base.info()["decode_grid"] == 148
         ws_default = B.csv_plan_workspace_bytes(sh, c5q, c5kv)
@@ -322,11 +322,23 @@ def test_tuning_knobs_are_read_at_plan_build_and_recorded_in_the_plan():
         B.csv_tuning_set(B.TUNE_DECODE_GRID, 37)
         assert B.Plan(sh, c5q, c5kv).info()["decode_grid"] == 37
         assert B.Plan(sh, [1], [16]).info()["decode_grid"] == 1         # a cap, not a floor
-        for bad in ((-1, 1), (3, 1), (0, -5), (1, (1 << 20) + 1)):
+        # the per-SM rates of the two roles are the caller's to calibrate: a device whose SMs stream faster needs fewer
+        # decode-role CTAs for the same step, one whose tensor pipes are faster needs more
+        c3 = synth.config_lengths(3)
+        sh8 = B.attn_shape(32, 8, 128)
+        k_default = B.Plan(sh8, c3["q_lens"], c3["kv_lens"]).info()["tail_n_dec"]
+        B.csv_tuning_set(B.TUNE_SM_DECODE_GBS, 100)
+        k_fast_hbm = B.Plan(sh8, c3["q_lens"], c3["kv_lens"]).info()["tail_n_dec"]
+        B.csv_tuning_set(B.TUNE_SM_DECODE_GBS, 0)
+        B.csv_tuning_set(B.TUNE_SM_APPEND_GFLOPS, 14800)
+        k_fast_mma = B.Plan(sh8, c3["q_lens"], c3["kv_lens"]).info()["tail_n_dec"]
+        B.csv_tuning_set(B.TUNE_SM_APPEND_GFLOPS, 0)
+        assert 0 < k_fast_hbm < k_default < k_fast_mma
+        for bad in ((-1, 1), (5, 1), (0, -5), (1, (1 << 20) + 1)):
             with pytest.raises(B.CsvError):
                 B.csv_tuning_set(*bad)
     finally:
-        for k in (0, 1, 2):
+        for k in range(5):
             B.csv_tuning_set(k, 0)
     assert B.Plan(sh, c5q, c5kv).info()["decode_grid"] == 148
 
