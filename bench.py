@@ -52,7 +52,8 @@ METRIC = "paged_decode_attn_hbm_gbs"
 UNIT = "GB/s"
 NOMINAL_HBM_GBS = 8000.0        # north_star's "~8 TB/s"; targets (70 % / 80 %) are stated against it
 O_TOL, LSE_TOL = 1e-2, 1e-3     # north_star's gates; the sampled rows of the timed configuration are checked live
-TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r2_traffic.csv")
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r3_traffic.csv")        # --ingest-ncu appends here (one file per round)
+TRAFFIC_CSVS = [os.path.join(ROOT, "profiles", "r2_traffic.csv"), TRAFFIC_CSV]   # read in this order: the latest row wins
 CSRC = os.path.join(ROOT, "paper_2606_01839_b200", "csrc")
 KERNEL_SOURCE = {"decode_kernel": "decode_attn.cu+decode_worker.cuh", "append_tc2_kernel": "append_attn_tc2.cu+append_tc2_body.cuh",
                  "pack_kernel": "handoff.cu", "unpack_kernel": "handoff.cu", "direct_kernel": "handoff.cu",
@@ -171,17 +172,19 @@ def sha256_of(files):
 
 
 def traffic_for(kernel, config):
-    """(dram read + write bytes per launch, provenance) from profiles/r2_traffic.csv — only if the capture was taken on
-    the kernel source as it is now (sha256 of the .cu file recorded at capture time); otherwise (None, why)."""
-    try:
-        rows = [l.rstrip("\n").split(",") for l in open(TRAFFIC_CSV) if l.strip() and not l.startswith("#")]
-    except Exception:
-        return None, "no capture (profiles/r2_traffic.csv absent)"
-    hdr, best = rows[0], None
-    for r in rows[1:]:
-        d = dict(zip(hdr, r))
-        if d["kernel"] == kernel and d["config"] == config:
-            best = d
+    """(dram read + write bytes per launch, provenance) from profiles/r2_traffic.csv + r3_traffic.csv — only if the capture
+    was taken on the kernel source as it is now (sha256 of the .cu file recorded at capture time); otherwise (None, why)."""
+    best = None
+    for path in TRAFFIC_CSVS:
+        try:
+            rows = [l.rstrip("\n").split(",") for l in open(path) if l.strip() and not l.startswith("#")]
+        except Exception:
+            continue
+        hdr = rows[0]
+        for r in rows[1:]:
+            d = dict(zip(hdr, r))
+            if d["kernel"] == kernel and d["config"] == config:
+                best = d
     if best is None:
         return None, "no capture for this (kernel, config)"
     cur = sha256_of(best["source_file"])
@@ -656,9 +659,99 @@ def leg_handoff(pk, iters=5):
             "payload_gb": payload / 1e9, "pack_ms": pack["median_ms"], "unpack_ms": unpack["median_ms"], "direct_ms": direct["median_ms"],
             "handoff_payload_gbs": {"pack_then_unpack": payload / (pack["median_ms"] + unpack["median_ms"]) / 1e6,
                                     "direct": payload / direct["median_ms"] / 1e6}}
+    # live parity of the three timed calls (bit-exact): sampled 64 KiB units (conversation, layer, block) against the oracle's
+    # staging message and scatter.  The pool is zeroed between the two routes so that neither can pass on the other's bits.
+    import oracle
+
+    oracle.build()
+    unit = 2 * Hkv * 16 * d
+    srng = np.random.default_rng(3003)
+    samples = []
+    for c in [int(np.argmin(toks)), int(np.argmax(toks))] + [int(x) for x in srng.integers(0, len(toks), size=4)]:
+        ntb = synth.blocks_for(toks[c])
+        samples += [(c, 0, 0), (c, NL - 1, ntb - 1)] + [(c, int(srng.integers(0, NL)), int(srng.integers(0, ntb))) for _ in range(4)]
+    u16 = lambda t: t.cpu().contiguous().numpy().view(np.uint16)
+
+    def units_match(staged):
+        bad = 0
+        for c, layer, tb in samples:
+            t = toks[c]
+            lo, hi = tb * 16, min(t, tb * 16 + 16)
+            K = u16(ks[c].view(NL, t, Hkv, d)[layer, lo:hi]).reshape(1, hi - lo, Hkv, d)
+            V = u16(vs[c].view(NL, t, Hkv, d)[layer, lo:hi]).reshape(1, hi - lo, Hkv, d)
+            if staged:   # the 64 KiB unit of the staging message, unused slots zero
+                msg = oracle.staging_message(1, Hkv, d, K, V, hi - lo, 0)
+                bad += int(not np.array_equal(u16(sts[c].view(NL, synth.blocks_for(t), unit)[layer, tb]), msg))
+            got = u16(d_pool.view(NL, nb, unit)[layer, int(ids[c][tb])])
+            want = oracle.scatter(np.zeros(unit, dtype=np.uint16), 1, 1, Hkv, d, K, V, hi - lo, 0, np.zeros(1, dtype=np.int32))
+            bad += int(not np.array_equal(got, want))
+        return bad
+
+    d_pool.zero_()
+    B.kv_pack_batch(desc, ks, vs, toks, offs, sts)
+    B.kv_unpack_batch(pool, sts, toks, offs, ids, nids)
+    torch.cuda.synchronize()
+    bad_staged = units_match(True)
+    d_pool.zero_()
+    B.kv_handoff_direct_batch(pool, ks, vs, toks, offs, ids, nids)
+    torch.cuda.synchronize()
+    bad_direct = units_match(False)
+    step["parity"] = {"what": "%d sampled 64 KiB units (conversation, layer, block) bit for bit against oracle.staging_message / "
+                              "oracle.scatter; pool zeroed between the routes" % len(samples),
+                      "kv_pack_batch + kv_unpack_batch mismatching units": bad_staged,
+                      "kv_handoff_direct_batch mismatching units": bad_direct, "ok": bool(bad_staged == 0 and bad_direct == 0)}
     del ks, vs, sts, d_pool
     torch.cuda.empty_cache()
     return blocks, [step]
+
+
+def leg_c1():
+    """BASELINE.json configs[0], the tiny correctness case (parity only, no roofline claim: everything is launch-bound): 4
+    conversations, Hq=4 Hkv=1 d=64, context U[64,512] in a shuffled paged pool, one decode row each through paged_decode_step,
+    the whole config against the oracle; plus the 300-token handoff (kv_pack -> kv_unpack, and kv_handoff_direct) into a
+    zeroed pool, the whole pool image against oracle.scatter."""
+    import torch
+    import oracle
+    from paper_2606_01839_b200 import binding as B
+    from paper_2606_01839_b200 import synth, workloads
+
+    oracle.build()
+    wl = workloads.config_tail_workload(1)
+    wl.d_out.fill_(0x7FC0)
+    wl.decode_step()
+    torch.cuda.synchronize()
+    dt, _, res = oracle_timed(wl, [(b, [0]) for b in range(len(wl.kv_lens))], 1)
+    eo, el = parity_of(wl, res)
+    t1 = time_calls(wl.decode_step, 20, 3)
+    NL, Hkv, d, tokens, nb = 1, 1, 64, 300, 256
+    desc = B.pool_desc(NL, nb, Hkv, d)
+    rng = np.random.default_rng(0)
+    K = synth.random_bits(rng, (NL, tokens, Hkv, d))
+    V = synth.random_bits(rng, (NL, tokens, Hkv, d))
+    dk, dv = (torch.from_numpy(a.view(np.int16)).cuda() for a in (K, V))
+    ok = {}
+    for route in ("kv_pack + kv_unpack", "kv_handoff_direct"):
+        d_pool = torch.zeros(B.kv_pool_bytes(desc) // 2, dtype=torch.int16, device="cuda")
+        pool = B.KvPool(desc, d_pool)
+        pool.set_free_order(synth.shuffled_free_order(np.random.default_rng(1), nb))
+        ids = pool.alloc_blocks(synth.blocks_for(tokens))
+        d_ids = torch.from_numpy(ids).cuda()
+        if route.startswith("kv_pack"):
+            st = torch.empty(B.kv_staging_bytes(desc, tokens) // 2, dtype=torch.int16, device="cuda")
+            B.kv_pack(desc, dk, dv, tokens, 0, st)
+            B.kv_unpack(pool, st, tokens, 0, d_ids, len(ids))
+        else:
+            B.kv_handoff_direct(pool, dk, dv, tokens, 0, d_ids, len(ids))
+        torch.cuda.synchronize()
+        want = oracle.scatter(np.zeros(oracle.pool_elems(NL, nb, Hkv, d), dtype=np.uint16), NL, nb, Hkv, d, K, V, tokens, 0, ids)
+        ok[route] = bool(np.array_equal(d_pool.cpu().numpy().view(np.uint16), want))
+    step = {"config": "configs[0]", "what": "tiny correctness case: 4 decode rows (Hq=4 Hkv=1 d=64, context U[64,512]) through "
+            "paged_decode_step + a 300-token handoff; parity only (launch-bound: no roofline claim)",
+            "ms_median": t1["median_ms"], "oracle_whole_config_seconds": dt,
+            "parity": {"paged_decode_step max_abs_err_O": eo, "paged_decode_step max_abs_err_LSE": el,
+                       "handoff whole pool image bit-exact": ok,
+                       "ok": bool(eo <= O_TOL and el <= LSE_TOL and all(ok.values()))}}
+    return [], [step]
 
 
 def leg_prefill(pk, iters=4):
@@ -716,7 +809,7 @@ def run_only(args):
 
 
 def ingest_ncu(args):
-    """profiles/r2_traffic.csv += one row: mean dram read / write bytes per launch of `--kernel` in an .ncu-rep."""
+    """profiles/r3_traffic.csv += one row: mean dram read / write bytes per launch of `--kernel` in an .ncu-rep."""
     txt = subprocess.run(["ncu", "-i", args.ingest_ncu, "--page", "raw", "--csv"], capture_output=True, text=True, check=True).stdout
     import csv
     import io
@@ -740,7 +833,7 @@ def ingest_ncu(args):
     with open(TRAFFIC_CSV, "a") as f:
         if new:
             f.write("# dram__bytes_read.sum / dram__bytes_write.sum per launch (mean over the captured launches) of `ncu --set full` "
-                    "captures; written by `python bench.py --ingest-ncu REP --kernel K --config C` (commands: profiles/r2_README.md).\n"
+                    "captures; written by `python bench.py --ingest-ncu REP --kernel K --config C` (commands: profiles/r3_README.md).\n"
                     "# bench.py reports a row as roofline.traffic only while sha256 over the csrc files named in source_file still equals source_sha256.\n")
             f.write("kernel,config,dram_read_bytes,dram_write_bytes,launches,commit,source_file,source_sha256,report\n")
         f.write("%s,%s,%.0f,%.0f,%d,%s,%s,%s,%s\n" % (args.kernel, args.config, rd / n, wr / n, n, commit, src,
@@ -937,12 +1030,18 @@ def run_ours(args):
         del wl
         torch.cuda.empty_cache()
         if not args.no_extras:
-            for name, fn in (("c2", lambda: leg_c2(args, pk, dist, agg_dev)), ("c3", lambda: leg_c3(args, pk, True)),
+            for name, fn in (("c1", lambda: leg_c1() + (None,)), ("c2", lambda: leg_c2(args, pk, dist, agg_dev)),
+                             ("c3", lambda: leg_c3(args, pk, True)),
                              ("handoff", lambda: leg_handoff(pk) + (None,)), ("prefill", lambda: leg_prefill(pk) + (None,))):
                 r = guarded(name, fn)
                 if r:
                     rooflines += r[0]
                     steps += r[1]
+                    for st in r[1]:   # legs whose parity is bit-exact work (handoff) or a whole tiny config carry it in their step
+                        if isinstance(st.get("parity"), dict):
+                            line["parity"]["routes"].append({"route": st["config"] + ": " + st["parity"].get("what", st["what"])[:160],
+                                                             "ok": st["parity"]["ok"]})
+                            line["parity"]["ok"] = bool(line["parity"]["ok"] and st["parity"]["ok"])
                     if len(r) > 2 and r[2]:
                         line["parity"]["routes"] += r[2].pop("parity_routes", [])
                         cpus.append(r[2])

@@ -26,7 +26,8 @@ struct AppendTc2Params {
     float* pml;
     int32_t max_blocks, Hq, Hkv, G;
     float scale_log2;
-    uint32_t* sched;   // [0] next item of the work queue (beyond the first gridDim.x), [1] CTAs that have finished
+    uint32_t* sched;   // [0] next item of the work queue (beyond the first gridDim.x), [1] unused, [2] next decode share of
+                       // tail_kernel; zeroed by the launcher (cudaMemsetAsync) before every launch
 };
 
 constexpr uint32_t kOffQ2 = 0;                           // 2 tiles x [2 halves][128 rows][128 B]

@@ -8,8 +8,9 @@
 //     that claims share s runs the 8 warp-workers of decode_worker.cuh on workers [8 s, 8 s + 8) (private 3-stage rings);
 //   append ITEMS: the longest-first item list of the two-tile tcgen05 body (append_tc2_body.cuh).
 // The first `n_dec` CTAs start on decode shares, the others on append items, and a CTA whose own queue is empty takes work
-// from the other one, so the split chosen by the plan (from the two roles' measured per-SM rates: HBM saturates with about
-// half of the SMs streaming, 61-79 GB/s per SM) only has to be roughly right and every share is processed whichever CTAs
+// from the other one, so the split chosen by the plan (from the two roles' measured per-SM rates, 61-79 GB/s per SM in the
+// decode role; HBM saturates near three quarters of the SMs streaming, which is where plan_tail caps the decode side) only
+// has to be roughly right and every share is processed whichever CTAs
 // run.  (Choosing the decode SMs evenly by SM id instead of by CTA index was measured and is slower: 4.94 against 4.64 ms
 // on configs[2].)  Why roles per SM and not both kinds on every SM: the append CTA leaves
 // 4 K registers and 30 KB of shared memory on its SM (measured: a co-resident decode CTA would have to fit in 64 registers

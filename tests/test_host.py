@@ -409,7 +409,7 @@ def test_tail_step_host_refuses_bad_lengths_before_any_copy_is_enqueued():
 
 def test_committed_ncu_traffic_rows_belong_to_the_current_kernel_sources():
     # bench.py reports roofline.traffic only from a capture taken on the kernel sources as they are now (sha256 recorded at
-    # ingest time in profiles/r2_traffic.csv).  A kernel edit without a fresh capture must show up here, not as a silent null.
+    # ingest time in profiles/r2_traffic.csv / r3_traffic.csv).  A kernel edit without a fresh capture must show up here, not as a silent null.
     import importlib.util
     import os
 
