@@ -474,6 +474,15 @@ def leg_c2(args, pk, dist, agg_dev):
     g = None if args.no_graph else graph_of(wl.decode_step)
     st = time_calls(g.replay if g else wl.decode_step, 100, 5)
     dec = time_calls(wl.decode, 100, 5)
+    # the same call without a plan or a workspace (paged_decode_attn_static: host plan + list upload into the library's
+    # static scratch array on every call, then the same kernels), for callers that cannot allocate device memory
+    stat_out, stat_lse = torch.empty_like(wl.d_out), torch.empty_like(wl.d_lse)
+    static_call = lambda: B.paged_decode_attn_static(wl.pool, 0, wl.shape, wl.kv_lens, wl.d_q, wl.d_tables, wl.max_blocks,
+                                                     stat_out, stat_lse)
+    stat = time_calls(static_call, 100, 5)
+    wl.decode()
+    torch.cuda.synchronize()
+    static_same = bool(torch.equal(stat_out, wl.d_out) and torch.equal(stat_lse, wl.d_lse))
     pin = lambda t: t.cpu().pin_memory()
     h_q, h_k, h_v = pin(wl.d_q), pin(wl.d_k_new), pin(wl.d_v_new)
     h_t = torch.from_numpy(wl.h_tables).pin_memory()
@@ -507,7 +516,11 @@ def leg_c2(args, pk, dist, agg_dev):
                         "per step while the H2D copies fly)",
             "h2d_bytes": (h_q.numel() + h_k.numel() + h_v.numel()) * 2 + h_t.numel() * 4,
             "d2h_bytes": h_out.numel() * 2 + h_lse.numel() * 4, "plan_host_us": sorted(pt)[len(pt) // 2],
-            "decode_items": info["n_decode_items"]}
+            "decode_items": info["n_decode_items"],
+            "static_scratch_call_ms": stat["median_ms"], "plan_and_workspace_call_ms": dec["median_ms"],
+            "static_scratch_what": "paged_decode_attn_static (no plan, no workspace: plans on the host and uploads the lists into "
+                                   "the library's 8 MiB static array on every call) against paged_decode_attn on a prebuilt plan; "
+                                   "CUDA events around the call", "static_scratch_bit_identical": static_same}
     block = roofline_block("decode_kernel", "configs[1]", "hbm", kv_bytes, dec, pk,
                            note="per paged_decode_attn call (decode_kernel + decode_merge_kernel)")
     # The WHOLE config through the oracle on one core ("c1, c2: the whole config"), timed, and compared with the
@@ -517,7 +530,8 @@ def leg_c2(args, pk, dist, agg_dev):
     wl.decode_step()
     torch.cuda.synchronize()
     dt, th, res = oracle_timed(wl, [(b, [0]) for b in range(rows)], 1)
-    routes = [route_record("paged_decode_step, configs[1], whole config (64 conversations x 32 heads)", *parity_of(wl, res))]
+    routes = [route_record("paged_decode_step, configs[1], whole config (64 conversations x 32 heads)", *parity_of(wl, res)),
+              route_record("paged_decode_attn_static, configs[1], whole config", *parity_of(wl, res, stat_out, stat_lse))]
     last = big.with_q_lens([1] * rows, kv_lens=[t + 104 for t in base])
     last.d_q.copy_(wl.d_q)
     _, _, res_last = oracle_timed(last, [(b, [0]) for b in range(0, rows, 8)], 1)
