@@ -18,6 +18,9 @@
  *  - The library NEVER allocates device memory. "d_" arguments are device
  *    pointers owned by the caller (e.g. torch tensors' data_ptr()); "h_"
  *    arguments are host pointers. `stream` is a cudaStream_t passed as void*.
+ *    (The one piece of device memory that is the library's own is the fixed
+ *    CSV_STATIC_SCRATCH_BYTES array behind paged_decode_attn_static: part of
+ *    the loaded image, not an allocation; see that call for what it costs.)
  *  - Kernel-launching calls enqueue on `stream` and return without
  *    synchronising. Host-side calls (allocator, plan, place) are synchronous,
  *    thread-compatible, not thread-safe.
